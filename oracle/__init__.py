@@ -1,0 +1,143 @@
+"""CPU oracle -- TEST INFRASTRUCTURE, not the product.
+
+Thin ctypes access to ``oracle/pdf_oracle.c`` (plain scalar C, fp64).  Only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
+legs may import this package.  It imports nothing from ``paper_2009_06635_b200``.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "pdf_oracle.c")
+_LIB = os.path.join(_HERE, "libpdforacle.so")
+_lib = None
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int)
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with gcc (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-Wall",
+               "-o", _LIB, _SRC, "-lquadmath", "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        lib.oracle_pdf_grid_create.restype = ctypes.c_void_p
+        lib.oracle_pdf_grid_create.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _ip, _dp,
+                                               ctypes.c_int, _ip, _dp]
+        lib.oracle_pdf_grid_free.argtypes = [ctypes.c_void_p]
+        lib.oracle_pdf_grid_invalid.restype = ctypes.c_long
+        lib.oracle_pdf_grid_invalid.argtypes = [ctypes.c_void_p]
+        lib.oracle_pdf_xfxq2.restype = ctypes.c_int
+        lib.oracle_pdf_xfxq2.argtypes = [ctypes.c_void_p, ctypes.c_int, _ip, ctypes.c_long,
+                                         _dp, _dp, _dp, _dp]
+        lib.oracle_alphas_create.restype = ctypes.c_void_p
+        lib.oracle_alphas_create.argtypes = [ctypes.c_int, _dp, _dp]
+        lib.oracle_alphas_free.argtypes = [ctypes.c_void_p]
+        lib.oracle_alphas_q2.restype = ctypes.c_int
+        lib.oracle_alphas_q2.argtypes = [ctypes.c_void_p, ctypes.c_long, _dp, _dp]
+        lib.oracle_ln.restype = ctypes.c_double
+        lib.oracle_ln.argtypes = [ctypes.c_double]
+        lib.oracle_threads.restype = ctypes.c_int
+        lib.oracle_set_threads.argtypes = [ctypes.c_int]
+        _lib = lib
+    return _lib
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def threads() -> int:
+    return int(_load().oracle_threads())
+
+
+def set_threads(n: int) -> None:
+    _load().oracle_set_threads(int(n))
+
+
+def ln(a: float) -> float:
+    return float(_load().oracle_ln(float(a)))
+
+
+class OraclePdfGrid:
+    """Oracle-side grid (arguments as in the C-ABI's pdf_grid_load)."""
+
+    def __init__(self, x_knots, q_offsets, q_knots, pids, values):
+        lib = _load()
+        x_knots, q_knots, values = _f64(x_knots), _f64(q_knots), _f64(values)
+        q_offsets, pids = _i32(q_offsets), _i32(pids)
+        self._h = lib.oracle_pdf_grid_create(
+            len(q_offsets) - 1, len(x_knots), x_knots.ctypes.data_as(_dp),
+            q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
+            pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp))
+
+    @classmethod
+    def from_spec(cls, spec):
+        return cls(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, spec.values)
+
+    def xfxq2(self, pids, x, q2, with_scale: bool = False):
+        """-> out[n_req, n] (flavour-major); with_scale also returns the conditioning scale."""
+        lib = _load()
+        pids, x, q2 = _i32(np.atleast_1d(pids)), _f64(np.atleast_1d(x)), _f64(np.atleast_1d(q2))
+        assert x.shape == q2.shape and x.ndim == 1
+        n = x.shape[0]
+        out = np.empty((len(pids), n), dtype=np.float64)
+        scale = np.empty_like(out) if with_scale else None
+        rc = lib.oracle_pdf_xfxq2(self._h, len(pids), pids.ctypes.data_as(_ip), n,
+                                  x.ctypes.data_as(_dp), q2.ctypes.data_as(_dp),
+                                  out.ctypes.data_as(_dp),
+                                  scale.ctypes.data_as(_dp) if with_scale else None)
+        if rc != 0:
+            raise ValueError(f"oracle_pdf_xfxq2 failed with {rc} (requested PID absent?)")
+        return (out, scale) if with_scale else out
+
+    @property
+    def n_invalid(self) -> int:
+        return int(_load().oracle_pdf_grid_invalid(self._h))
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.oracle_pdf_grid_free(self._h)
+            self._h = None
+
+
+class OracleAlphas:
+    def __init__(self, q_knots, alphas):
+        lib = _load()
+        q_knots, alphas = _f64(q_knots), _f64(alphas)
+        assert q_knots.shape == alphas.shape
+        self._h = lib.oracle_alphas_create(len(q_knots), q_knots.ctypes.data_as(_dp),
+                                           alphas.ctypes.data_as(_dp))
+
+    @classmethod
+    def from_spec(cls, spec):
+        return cls(spec.q_knots, spec.alphas)
+
+    def q2(self, q2):
+        lib = _load()
+        q2 = _f64(np.atleast_1d(q2))
+        out = np.empty_like(q2)
+        lib.oracle_alphas_q2(self._h, q2.shape[0], q2.ctypes.data_as(_dp), out.ctypes.data_as(_dp))
+        return out
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.oracle_alphas_free(self._h)
+            self._h = None
