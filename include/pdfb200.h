@@ -1,0 +1,129 @@
+/*
+ * pdfb200.h -- C-ABI of libpdfb200: batched parton-distribution and alpha_s interpolation
+ * on one NVIDIA B200 (sm_100a), fp64.
+ *
+ * What the library computes is the hot path of PDFFlow (arXiv:2009.06635; citations are
+ * lines of PAPER.md): "a log-bicubic PDF interpolation in terms of x and Q^2" following the
+ * LHAPDF6 prescription, on Q^2 sub-grids that are interpolated independently, with one-sided
+ * rules "close to quark mass thresholds and grids x edges" (section 2.2), and
+ * "a log-cubic interpolation with constant extrapolation from the (alpha_s(Q), Q) nodes",
+ * sub-grid aware (section 2.3).  The exact formulas (readings O1-O6) are stated
+ * in DESIGN.md; the paper prints none.
+ *
+ * Conventions
+ *   - Every call returns an int: PDFB_OK (0) or a negative PDFB_E* code; pdfb_strerror()
+ *     gives text.  No C++ exception crosses this boundary.
+ *   - "host" / "device" on a pointer says where the memory lives.  Device pointers must
+ *     belong to the device the handle was loaded on.
+ *   - Handles own all device memory they allocate until *_free().  *_load() copies its host
+ *     arrays; the caller may free them immediately.
+ *   - Evaluation calls with device pointers allocate nothing, never synchronise and only
+ *     enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).
+ *   - There is no CPU fallback: without a CUDA device *_load() fails with PDFB_ECUDA.
+ */
+#ifndef PDFB200_H
+#define PDFB200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pdfb_grid pdfb_grid;     /* opaque; PDF knot grid on one device   */
+typedef struct pdfb_alphas pdfb_alphas; /* opaque; alpha_s node list on one device */
+
+enum {
+    PDFB_OK = 0,
+    PDFB_EINVAL = -1,   /* null pointer, negative size, bad count                       */
+    PDFB_EKNOTS = -2,   /* knots not strictly increasing / non-positive / subgrids do not
+                           share their threshold knot / a subgrid has < 2 Q knots        */
+    PDFB_EPID = -3,     /* requested PID not in the grid (PID 0 is an alias of 21)       */
+    PDFB_ECUDA = -4,    /* CUDA runtime error (no device, out of memory, launch failure) */
+    PDFB_ELIMIT = -5    /* more than PDFB_MAX_SUBGRIDS subgrids or PDFB_MAX_PIDS PIDs    */
+};
+#define PDFB_MAX_SUBGRIDS 16
+#define PDFB_MAX_PIDS 32
+
+/*
+ * pdf_grid_load -- upload one PDF member's knot grid and run the grid-setup kernel
+ * (reading O2: finite-difference derivative rule, one-sided at x edges and at sub-grid
+ * edges).
+ *
+ *   n_sub      number of Q^2 sub-grids, >= 1
+ *   nx         number of x knots (shared by all sub-grids), >= 2
+ *   x_knots    host [nx], strictly increasing, > 0
+ *   q_offsets  host [n_sub+1], q_offsets[0] = 0; sub-grid s owns q_knots[q_offsets[s] ..
+ *              q_offsets[s+1]), at least 2 knots each
+ *   q_knots    host [q_offsets[n_sub]], Q in GeV (not Q^2), strictly increasing inside a
+ *              sub-grid; the last knot of sub-grid s equals the first of s+1 (the threshold)
+ *   n_pid,pids host [n_pid], PDG ids of the value columns (e.g. -5..5 and 21)
+ *   values     host, xf at the knots, layout [s][ix][iq][ipid] row-major with the sub-grids
+ *              concatenated (LHAPDF grid-file order)
+ *   device     CUDA device ordinal
+ *   out        receives the handle
+ */
+int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
+                  const double *q_knots, int n_pid, const int *pids, const double *values,
+                  int device, pdfb_grid **out);
+
+/*
+ * pdf_xfxq2 -- xf_pid(x, Q^2) for n points and n_req flavours (section 2.2;
+ * readings O3-O5).  Points outside the grid are continued (x < x_min, Q^2 outside
+ * [q_min, q_max]); points with no value (x > x_max, x <= 0, Q^2 <= 0, NaN, Inf) give NaN in
+ * every flavour and are counted (pdf_grid_status).
+ *
+ *   pids   host [n_req]; each must be in the grid (else PDFB_EPID, nothing is launched)
+ *   x, q2  device [n], fp64, read-only
+ *   out    device [n_req][n], flavour-major: out[r*n + p] = xf of pids[r] at point p
+ */
+int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+              const double *q2, double *out, void *cuda_stream);
+
+/*
+ * pdf_xfxq2_host -- the same for HOST buffers (pinned or pageable): chunks are copied to the
+ * device, evaluated and copied back on internal streams, overlapping the three stages.
+ * Synchronous: returns when `out` is complete.  Staging buffers are owned by the handle.
+ */
+int pdf_xfxq2_host(pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                   const double *q2, double *out);
+
+/* Number of points so far that had no value (synchronises the device; sticky counter). */
+int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points);
+
+/* Device time of the grid-setup kernels of this handle's pdf_grid_load, in ms (-1 on NULL). */
+double pdf_grid_setup_ms(const pdfb_grid *g);
+
+void pdf_grid_free(pdfb_grid *g);
+
+/*
+ * alphas_grid_load -- upload the (Q_k, alpha_s(Q_k)) nodes.
+ *   q_knots  host [n_knots], Q in GeV, non-decreasing, > 0; a repeated value marks a flavour
+ *            threshold and splits the list into sub-grids (the two copies may carry
+ *            different alpha_s); every sub-grid needs >= 2 nodes
+ *   alphas   host [n_knots]
+ */
+int alphas_grid_load(int n_knots, const double *q_knots, const double *alphas, int device,
+                     pdfb_alphas **out);
+
+/*
+ * alphas_q2 -- alpha_s(Q^2) for n points (reading O6): cubic Hermite in ln Q^2 inside the
+ * node range with one-sided derivatives at sub-grid edges, frozen at the first / last node
+ * value outside ("constant extrapolation").  Q^2 <= 0 or NaN gives NaN.
+ *   q2, out  device [n]
+ */
+int alphas_q2(const pdfb_alphas *a, long long n, const double *q2, double *out,
+              void *cuda_stream);
+
+/* alphas_q2 for HOST buffers; synchronous. */
+int alphas_q2_host(pdfb_alphas *a, long long n, const double *q2, double *out);
+
+void alphas_grid_free(pdfb_alphas *a);
+
+const char *pdfb_strerror(int code);
+
+/* Kernels launched by this library since load (all handles); for bench accounting. */
+long long pdfb_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDFB200_H */

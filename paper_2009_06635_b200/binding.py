@@ -1,0 +1,202 @@
+"""Thin ctypes binding of include/pdfb200.h -- argument marshalling only.
+
+Same names as the C-ABI.  Host arrays are numpy; device arrays are torch CUDA tensors (torch
+supplies device memory and streams, nothing else).  There is no fallback: if libpdfb200.so is
+missing or does not load, ``lib()`` raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpdfb200.so")
+_lib = None
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int)
+_vp = ctypes.c_void_p
+_ll = ctypes.c_longlong
+
+EXPORTS = ("pdf_grid_load", "pdf_xfxq2", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
+           "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
+           "pdfb_launch_count")
+
+
+class PdfbError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {strerror(code)} (code {code})")
+
+
+def lib():
+    """Load libpdfb200.so (built in-tree by ``paper_2009_06635_b200.build``); fail loudly."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2009_06635_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.pdf_grid_load.restype = ctypes.c_int
+        L.pdf_grid_load.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _ip, _dp, ctypes.c_int, _ip, _dp,
+                                    ctypes.c_int, ctypes.POINTER(_vp)]
+        L.pdf_xfxq2.restype = ctypes.c_int
+        L.pdf_xfxq2.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
+        L.pdf_xfxq2_host.restype = ctypes.c_int
+        L.pdf_xfxq2_host.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp]
+        L.pdf_grid_status.restype = ctypes.c_int
+        L.pdf_grid_status.argtypes = [_vp, ctypes.POINTER(_ll)]
+        L.pdf_grid_free.restype = None
+        L.pdf_grid_free.argtypes = [_vp]
+        L.pdf_grid_setup_ms.restype = ctypes.c_double
+        L.pdf_grid_setup_ms.argtypes = [_vp]
+        L.alphas_grid_load.restype = ctypes.c_int
+        L.alphas_grid_load.argtypes = [ctypes.c_int, _dp, _dp, ctypes.c_int, ctypes.POINTER(_vp)]
+        L.alphas_q2.restype = ctypes.c_int
+        L.alphas_q2.argtypes = [_vp, _ll, _vp, _vp, _vp]
+        L.alphas_q2_host.restype = ctypes.c_int
+        L.alphas_q2_host.argtypes = [_vp, _ll, _vp, _vp]
+        L.alphas_grid_free.restype = None
+        L.alphas_grid_free.argtypes = [_vp]
+        L.pdfb_strerror.restype = ctypes.c_char_p
+        L.pdfb_strerror.argtypes = [ctypes.c_int]
+        L.pdfb_launch_count.restype = _ll
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().pdfb_strerror(int(code)).decode()
+
+
+def launch_count() -> int:
+    return int(lib().pdfb_launch_count())
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i32(a):
+    return np.ascontiguousarray(np.atleast_1d(a), dtype=np.int32)
+
+
+def _check(rc: int, where: str):
+    if rc != 0:
+        raise PdfbError(rc, where)
+
+
+def _dev_ptr(t, n, name):
+    """Pointer of a contiguous float64 CUDA tensor with at least n elements."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous float64 CUDA tensor")
+    if t.numel() < n:
+        raise ValueError(f"{name} has {t.numel()} elements, need {n}")
+    return ctypes.c_void_p(t.data_ptr())
+
+
+def _host_ptr(a, n, name):
+    """Pointer of host memory: numpy float64 array or CPU (possibly pinned) torch tensor."""
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float64 or not a.flags.c_contiguous or a.size < n:
+            raise TypeError(f"{name} must be a C-contiguous float64 array with >= {n} elements")
+        return ctypes.c_void_p(a.ctypes.data)
+    import torch
+    if isinstance(a, torch.Tensor) and not a.is_cuda and a.dtype == torch.float64 and a.is_contiguous() \
+            and a.numel() >= n:
+        return ctypes.c_void_p(a.data_ptr())
+    raise TypeError(f"{name} must be host float64 memory with >= {n} elements")
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, int):
+        return ctypes.c_void_p(stream)
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+# ------------------------------------------------------------------ the C-ABI calls
+def pdf_grid_load(x_knots, q_offsets, q_knots, pids, values, device: int = 0):
+    """-> opaque handle (int).  Arguments as in pdfb200.h; host numpy arrays."""
+    x_knots, q_knots, values = _f64(x_knots), _f64(q_knots), _f64(values)
+    q_offsets, pids = _i32(q_offsets), _i32(pids)
+    h = _vp()
+    rc = lib().pdf_grid_load(len(q_offsets) - 1, len(x_knots), x_knots.ctypes.data_as(_dp),
+                             q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
+                             pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp), int(device),
+                             ctypes.byref(h))
+    _check(rc, "pdf_grid_load")
+    return h.value
+
+
+def pdf_xfxq2(g, pids, x, q2, out, stream=None, n=None):
+    """Enqueue xf(x,Q^2) for device tensors x, q2 -> out[n_req, n] on `stream` (torch current)."""
+    pids = _i32(pids)
+    n = int(x.numel() if n is None else n)
+    rc = lib().pdf_xfxq2(_vp(g), len(pids), pids.ctypes.data_as(_ip), n, _dev_ptr(x, n, "x"),
+                         _dev_ptr(q2, n, "q2"), _dev_ptr(out, len(pids) * n, "out"), _stream_ptr(stream))
+    _check(rc, "pdf_xfxq2")
+
+
+def pdf_xfxq2_host(g, pids, x, q2, out):
+    """Synchronous evaluation for HOST buffers (numpy or pinned torch CPU tensors)."""
+    pids = _i32(pids)
+    n = int(x.size if isinstance(x, np.ndarray) else x.numel())
+    rc = lib().pdf_xfxq2_host(_vp(g), len(pids), pids.ctypes.data_as(_ip), n, _host_ptr(x, n, "x"),
+                              _host_ptr(q2, n, "q2"), _host_ptr(out, len(pids) * n, "out"))
+    _check(rc, "pdf_xfxq2_host")
+
+
+def pdf_grid_status(g) -> int:
+    c = _ll(0)
+    _check(lib().pdf_grid_status(_vp(g), ctypes.byref(c)), "pdf_grid_status")
+    return int(c.value)
+
+
+def pdf_grid_setup_ms(g) -> float:
+    return float(lib().pdf_grid_setup_ms(_vp(g)))
+
+
+def pdf_grid_free(g):
+    lib().pdf_grid_free(_vp(g))
+
+
+def alphas_grid_load(q_knots, alphas, device: int = 0):
+    q_knots, alphas = _f64(q_knots), _f64(alphas)
+    if q_knots.shape != alphas.shape:
+        raise ValueError("q_knots and alphas differ in length")
+    h = _vp()
+    rc = lib().alphas_grid_load(len(q_knots), q_knots.ctypes.data_as(_dp), alphas.ctypes.data_as(_dp),
+                                int(device), ctypes.byref(h))
+    _check(rc, "alphas_grid_load")
+    return h.value
+
+
+def alphas_q2(a, q2, out, stream=None, n=None):
+    n = int(q2.numel() if n is None else n)
+    rc = lib().alphas_q2(_vp(a), n, _dev_ptr(q2, n, "q2"), _dev_ptr(out, n, "out"), _stream_ptr(stream))
+    _check(rc, "alphas_q2")
+
+
+def alphas_q2_host(a, q2, out):
+    n = int(q2.size if isinstance(q2, np.ndarray) else q2.numel())
+    rc = lib().alphas_q2_host(_vp(a), n, _host_ptr(q2, n, "q2"), _host_ptr(out, n, "out"))
+    _check(rc, "alphas_q2_host")
+
+
+def alphas_grid_free(a):
+    lib().alphas_grid_free(_vp(a))
+
+
+# ------------------------------------------------------------------ spec conveniences
+def load_pdf_spec(spec, device: int = 0):
+    return pdf_grid_load(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, spec.values, device)
+
+
+def load_alphas_spec(spec, device: int = 0):
+    return alphas_grid_load(spec.q_knots, spec.alphas, device)

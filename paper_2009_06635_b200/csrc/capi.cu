@@ -1,0 +1,205 @@
+// capi.cu -- the C-ABI of include/pdfb200.h: validation, host grid manager, handles.
+#include <atomic>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "pdfb_internal.cuh"
+
+static std::atomic<long long> g_launches{0};
+void pdfb_count_launch(int n) { g_launches += n; }
+extern "C" long long pdfb_launch_count(void) { return g_launches.load(); }
+
+extern "C" const char *pdfb_strerror(int code)
+{
+    switch (code) {
+    case PDFB_OK: return "ok";
+    case PDFB_EINVAL: return "invalid argument (null pointer, negative size or bad count)";
+    case PDFB_EKNOTS: return "bad knots (not increasing, non-positive, sub-grids not sharing their threshold, or < 2 knots)";
+    case PDFB_EPID: return "requested PID is not in the grid";
+    case PDFB_ECUDA: return "CUDA runtime error (no device, out of memory or launch failure)";
+    case PDFB_ELIMIT: return "too many sub-grids, PIDs or alpha_s nodes";
+    default: return "unknown pdfb error code";
+    }
+}
+
+// ln of a coordinate knot (reading R-ln).  Host side.
+static double knot_ln(double a) { return std::log(a); }
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ------------------------------------------------------------------------------ PDF grid
+extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
+                             const double *q_knots, int n_pid, const int *pids, const double *values,
+                             int device, pdfb_grid **out)
+{
+    if (!out) return PDFB_EINVAL;
+    *out = nullptr;
+    if (!x_knots || !q_offsets || !q_knots || !pids || !values) return PDFB_EINVAL;
+    if (n_sub < 1 || nx < 2 || n_pid < 1 || q_offsets[0] != 0) return PDFB_EINVAL;
+    if (n_sub > PDFB_MAX_SUBGRIDS || n_pid > PDFB_MAX_PIDS) return PDFB_ELIMIT;
+    for (int i = 0; i < nx; i++) {
+        if (!(x_knots[i] > 0.0) || !std::isfinite(x_knots[i])) return PDFB_EKNOTS;
+        if (i && !(x_knots[i] > x_knots[i - 1])) return PDFB_EKNOTS;
+    }
+    for (int s = 0; s < n_sub; s++) {
+        int a = q_offsets[s], b = q_offsets[s + 1];
+        if (b - a < 2) return PDFB_EKNOTS;
+        for (int j = a; j < b; j++) {
+            if (!(q_knots[j] > 0.0) || !std::isfinite(q_knots[j])) return PDFB_EKNOTS;
+            if (j > a && !(q_knots[j] > q_knots[j - 1])) return PDFB_EKNOTS;
+        }
+        if (s && q_knots[a] != q_knots[a - 1]) return PDFB_EKNOTS;
+    }
+    const int nq_tot = q_offsets[n_sub];
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return PDFB_ECUDA;
+    PDFB_CUDA(cudaSetDevice(device));
+
+    pdfb_grid *g = new (std::nothrow) pdfb_grid();
+    if (!g) return PDFB_EINVAL;
+    memset(g, 0, sizeof(*g));
+    g->device = device;
+    GridDev &d = g->d;
+    d.n_sub = n_sub; d.nx = nx; d.n_pid = n_pid; d.nq_tot = nq_tot;
+    d.kpad = (n_pid + 1) & ~1;  // even number of doubles per knot: 16-byte aligned knots
+    memcpy(g->pids, pids, sizeof(int) * n_pid);
+
+    // host-side knot arrays: raw and ln
+    std::vector<double> h_q2(nq_tot), h_z(nx + nq_tot);
+    for (int i = 0; i < nx; i++) h_z[i] = knot_ln(x_knots[i]);
+    for (int j = 0; j < nq_tot; j++) {
+        h_q2[j] = q_knots[j] * q_knots[j];
+        h_z[nx + j] = knot_ln(h_q2[j]);
+    }
+    long long knots = 0;
+    for (int s = 0; s < n_sub; s++) {
+        d.q_off[s] = q_offsets[s];
+        d.v_off[s] = (int)knots;
+        d.q2_lo[s] = h_q2[q_offsets[s]];
+        knots += (long long)nx * (q_offsets[s + 1] - q_offsets[s]);
+    }
+    d.q_off[n_sub] = nq_tot;
+    d.x_min = x_knots[0]; d.x_max = x_knots[nx - 1];
+    d.q2_min = h_q2[0]; d.q2_max = h_q2[nq_tot - 1];
+    d.U0 = h_z[0]; d.U1 = h_z[1]; d.inv_dU01 = 1.0 / (h_z[1] - h_z[0]);
+    d.Va = h_z[nx + nq_tot - 2]; d.Vb = h_z[nx + nq_tot - 1]; d.inv_dVab = 1.0 / (d.Vb - d.Va);
+
+    // one device blob: [xk | q2k | z (ln knots) | xrec | qrec | val | raw values | counter]
+    size_t o_xk = 0;
+    size_t o_q2k = align_up(o_xk + sizeof(double) * nx, 128);
+    size_t o_z = align_up(o_q2k + sizeof(double) * nq_tot, 128);
+    size_t o_xrec = align_up(o_z + sizeof(double) * (nx + nq_tot), 128);
+    size_t o_qrec = align_up(o_xrec + sizeof(IntervalRec) * nx, 128);
+    size_t o_val = align_up(o_qrec + sizeof(IntervalRec) * nq_tot, 128);
+    size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad, 128);
+    size_t o_raw = align_up(o_cnt + 128, 128);
+    size_t total = o_raw + sizeof(double) * knots * n_pid;
+    char *blob = nullptr;
+    if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
+    g->blob = blob; g->blob_bytes = total;
+
+    int rc = PDFB_OK;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    do {
+        if (cudaMemcpy(blob + o_xk, x_knots, sizeof(double) * nx, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(blob + o_q2k, h_q2.data(), sizeof(double) * nq_tot, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(blob + o_z, h_z.data(), sizeof(double) * (nx + nq_tot), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(blob + o_raw, values, sizeof(double) * knots * n_pid, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemset(blob + o_cnt, 0, 128) != cudaSuccess) { rc = PDFB_ECUDA; break; }
+        cudaEventRecord(e0, 0);
+        // K1: interval records for the x knots and for each sub-grid's Q^2 knots
+        int xoff[2] = {0, nx};
+        rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec), 1, xoff, 0);
+        if (rc) break;
+        rc = pdfb_setup_records((const double *)(blob + o_z) + nx, (IntervalRec *)(blob + o_qrec), n_sub, d.q_off, 0);
+        if (rc) break;
+        // K1: value table re-layout, sub-grid by sub-grid
+        long long src = 0;
+        for (int s = 0; s < n_sub && !rc; s++) {
+            int nq = q_offsets[s + 1] - q_offsets[s];
+            rc = pdfb_setup_values((const double *)(blob + o_raw) + src,
+                                   (double *)(blob + o_val) + (long long)d.v_off[s] * d.kpad, nx, nq, n_pid, d.kpad, 0);
+            src += (long long)nx * nq * n_pid;
+        }
+        if (rc) break;
+        cudaEventRecord(e1, 0);
+        if (cudaDeviceSynchronize() != cudaSuccess) { rc = PDFB_ECUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        g->setup_ms = ms;
+        // rule C's second probe sits at the fixed scale 1.01 * q2_min: its v weights are constants
+        double qC = 1.01 * d.q2_min;
+        int nq0 = q_offsets[1];
+        if (!(qC < h_q2[nq0 - 1])) { rc = PDFB_EKNOTS; break; }
+        int jC = 0;
+        for (int m = 1; m <= nq0 - 2; m++) if (h_q2[m] <= qC) jC = m;
+        IntervalRec rC;
+        if (cudaMemcpy(&rC, blob + o_qrec + sizeof(IntervalRec) * jC, sizeof(rC), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = PDFB_ECUDA; break; }
+        d.jC = jC;
+        weights4(rC, (knot_ln(qC) - rC.z0) * rC.inv_dz, d.wvC);
+    } while (0);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (rc) { cudaFree(blob); delete g; return rc; }
+
+    d.xk = (const double *)(blob + o_xk);
+    d.q2k = (const double *)(blob + o_q2k);
+    d.xrec = (const IntervalRec *)(blob + o_xrec);
+    d.qrec = (const IntervalRec *)(blob + o_qrec);
+    d.val = (const double *)(blob + o_val);
+    d.n_invalid = (unsigned long long *)(blob + o_cnt);
+    *out = g;
+    return PDFB_OK;
+}
+
+static int resolve_cols(const pdfb_grid *g, int n_req, const int *pids, int *cols)
+{
+    if (n_req < 1 || n_req > PDFB_MAX_PIDS) return PDFB_EINVAL;
+    for (int r = 0; r < n_req; r++) {
+        int pid = pids[r] == 0 ? 21 : pids[r];
+        cols[r] = -1;
+        for (int k = 0; k < g->d.n_pid; k++) if (g->pids[k] == pid) cols[r] = k;
+        if (cols[r] < 0) return PDFB_EPID;
+    }
+    return PDFB_OK;
+}
+
+extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                         const double *q2, double *out, void *cuda_stream)
+{
+    if (!g || !pids || n < 0) return PDFB_EINVAL;
+    if (n > 0 && (!x || !q2 || !out)) return PDFB_EINVAL;
+    int cols[PDFB_MAX_PIDS];
+    int rc = resolve_cols(g, n_req, pids, cols);
+    if (rc) return rc;
+    return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points)
+{
+    if (!g || !n_invalid_points) return PDFB_EINVAL;
+    unsigned long long c = 0;
+    PDFB_CUDA(cudaSetDevice(g->device));
+    PDFB_CUDA(cudaDeviceSynchronize());
+    PDFB_CUDA(cudaMemcpy(&c, g->d.n_invalid, sizeof(c), cudaMemcpyDeviceToHost));
+    *n_invalid_points = (long long)c;
+    return PDFB_OK;
+}
+
+extern "C" void pdf_grid_free(pdfb_grid *g)
+{
+    if (!g) return;
+    cudaSetDevice(g->device);
+    cudaDeviceSynchronize();
+    for (int i = 0; i < 3; i++) {
+        if (g->streams[i]) cudaStreamDestroy(g->streams[i]);
+        if (g->ev_done[i]) cudaEventDestroy(g->ev_done[i]);
+    }
+    if (g->stage) cudaFree(g->stage);
+    if (g->blob) cudaFree(g->blob);
+    delete g;
+}

@@ -1,0 +1,78 @@
+// grid_setup.cu -- K1: the grid-setup kernels, run once per pdf_grid_load / alphas_grid_load.
+//
+// Reading O2 ("special care ... close to quark mass thresholds and
+// grids x edges, where the minimum number of knots required for bicubic interpolation is not
+// available"): the derivative at a knot is the one-sided slope at either end of the knot
+// array -- the x-knot array, or the Q^2 knots of ONE sub-grid -- and the plain mean of the two
+// one-sided slopes inside.  K1 turns that rule into per-interval coefficient records
+// (IntervalRec) so that a query only fetches Hermite coefficients, and re-lays the value
+// table out for the evaluation kernel.
+#include "pdfb_internal.cuh"
+
+// One thread per interval m of the knot array z[0..M-1] (natural logs of the knots).
+__global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *__restrict__ rec, int M)
+{
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= M - 1) {
+        if (m == M - 1) {  // pad entry so every knot index has a record; never used by a cell
+            IntervalRec r = {z[m], 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+            rec[m] = r;
+        }
+        return;
+    }
+    double dz = z[m + 1] - z[m];
+    IntervalRec r;
+    r.z0 = z[m];
+    r.inv_dz = 1.0 / dz;
+    if (m == 0) {  // one-sided: dz * d_m = y_{m+1} - y_m
+        r.aLm = 0.0; r.aL0 = -1.0; r.aL1 = 1.0;
+    } else {       // dz * d_m = 1/2 [ (y_{m+1}-y_m) + (dz/dz_left)(y_m - y_{m-1}) ]
+        double rho = dz / (z[m] - z[m - 1]);
+        r.aLm = -0.5 * rho; r.aL0 = 0.5 * (rho - 1.0); r.aL1 = 0.5;
+    }
+    if (m + 1 == M - 1) {
+        r.aH0 = -1.0; r.aH1 = 1.0; r.aHp = 0.0;
+    } else {       // dz * d_{m+1} = 1/2 [ (dz/dz_right)(y_{m+2}-y_{m+1}) + (y_{m+1}-y_m) ]
+        double rho = dz / (z[m + 2] - z[m + 1]);
+        r.aH0 = -0.5; r.aH1 = 0.5 * (1.0 - rho); r.aHp = 0.5 * rho;
+    }
+    rec[m] = r;
+}
+
+// values of one sub-grid: file order [ix][iq][ipid] -> [iq][ix][kpad], padding columns = 0
+__global__ void k1_relayout_values(const double *__restrict__ src, double *__restrict__ dst, int nx,
+                                   int nq, int n_pid, int kpad)
+{
+    long long tot = (long long)nx * nq * kpad;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
+         e += (long long)gridDim.x * blockDim.x) {
+        int k = (int)(e % kpad);
+        long long knot = e / kpad;
+        int ix = (int)(knot % nx), iq = (int)(knot / nx);
+        dst[e] = (k < n_pid) ? src[((long long)ix * nq + iq) * n_pid + k] : 0.0;
+    }
+}
+
+int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, int n_arrays, const int *h_off,
+                       cudaStream_t st)
+{
+    for (int a = 0; a < n_arrays; a++) {
+        int M = h_off[a + 1] - h_off[a];
+        k1_interval_records<<<(M + 127) / 128, 128, 0, st>>>(d_z + h_off[a], d_rec + h_off[a], M);
+        pdfb_count_launch(1);
+    }
+    PDFB_CUDA(cudaGetLastError());
+    return PDFB_OK;
+}
+
+int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
+                      cudaStream_t st)
+{
+    long long tot = (long long)nx * nq * kpad;
+    int blocks = (int)((tot + 255) / 256);
+    if (blocks > 1184) blocks = 1184;
+    k1_relayout_values<<<blocks, 256, 0, st>>>(d_src, d_dst, nx, nq, n_pid, kpad);
+    pdfb_count_launch(1);
+    PDFB_CUDA(cudaGetLastError());
+    return PDFB_OK;
+}

@@ -1,0 +1,110 @@
+// pdfb_internal.cuh -- device-side data layout shared by the library's own translation units.
+// (Nothing under oracle/ includes this file, and this file includes nothing from oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/pdfb200.h"
+
+// One record per knot interval [z_m, z_{m+1}] of a 1-D knot array (x knots, or the Q^2 knots
+// of one sub-grid).  Written once by the grid-setup kernel K1 (reading O2: finite-difference
+// derivative rule).  With h00,h10,h01,h11 the cubic Hermite basis at
+// t = (z - z0) * inv_dz, the interpolant on the interval is  sum_a w_a y_{m-1+a}  with
+//   w_0 = h10*aLm,  w_1 = h00 + h10*aL0 + h11*aH0,  w_2 = h01 + h10*aL1 + h11*aH1,  w_3 = h11*aHp
+// i.e. dz * (derivative at knot m)   = aLm*y_{m-1} + aL0*y_m + aL1*y_{m+1}
+//      dz * (derivative at knot m+1) = aH0*y_m + aH1*y_{m+1} + aHp*y_{m+2}
+// At the first (last) interval of the array aLm (aHp) is exactly 0 and the derivative is the
+// one-sided slope.
+struct __align__(16) IntervalRec {
+    double z0;      // ln of the lower knot
+    double inv_dz;  // 1 / (ln upper - ln lower)
+    double aLm, aL0, aL1;
+    double aH0, aH1, aHp;
+};
+static_assert(sizeof(IntervalRec) == 64, "IntervalRec must be 64 bytes");
+
+// the four 1-D weights of knots m-1..m+2 at in-interval coordinate t (see IntervalRec)
+__host__ __device__ __forceinline__ void weights4(const IntervalRec &r, double t, double w[4])
+{
+    double t2 = t * t, t3 = t2 * t;
+    double h01 = 3.0 * t2 - 2.0 * t3;
+    double h00 = 1.0 - h01;
+    double h11 = t3 - t2;
+    double h10 = h11 - t2 + t;
+    w[0] = h10 * r.aLm;
+    w[1] = fma(h11, r.aH0, fma(h10, r.aL0, h00));
+    w[2] = fma(h11, r.aH1, fma(h10, r.aL1, h01));
+    w[3] = h11 * r.aHp;
+}
+
+struct GridDev {
+    int n_sub, nx, n_pid, nq_tot;
+    int kpad;                          // doubles per knot in `val` (>= n_pid)
+    int q_off[PDFB_MAX_SUBGRIDS + 1];  // knot offsets of the sub-grids
+    int v_off[PDFB_MAX_SUBGRIDS];      // offset (in knots) of sub-grid s in `val`
+    double q2_lo[PDFB_MAX_SUBGRIDS];   // first Q^2 knot of each sub-grid
+    double x_min, x_max, q2_min, q2_max;
+    // continuation (readings O4/O5)
+    double U0, U1, inv_dU01;           // ln x_0, ln x_1, 1/(U1-U0)
+    double Va, Vb, inv_dVab;           // ln of the last two Q^2 knots, 1/(Vb-Va)
+    int jC;                            // interval of 1.01*q2_min in sub-grid 0
+    double wvC[4];                     // its four v weights (fixed per grid)
+    const double *xk;                  // [nx] x knots
+    const double *q2k;                 // [nq_tot] Q^2 knots
+    const IntervalRec *xrec;           // [nx-1]
+    const IntervalRec *qrec;           // [nq_tot]; entry q_off[s]+j = interval j of sub-grid s
+    const double *val;                 // [s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
+    unsigned long long *n_invalid;     // sticky counter
+};
+
+struct AlphasDev {
+    int K, n_sub;
+    int off[PDFB_MAX_SUBGRIDS + 1];
+    double q2_lo[PDFB_MAX_SUBGRIDS];
+    double q2_min, q2_max, a_first, a_last;
+    const double *q2k;        // [K]
+    const double *a;          // [K]
+    const IntervalRec *rec;   // [K]
+};
+
+struct pdfb_grid {
+    int device;
+    GridDev d;
+    int pids[PDFB_MAX_PIDS];
+    void *blob;               // one device allocation holding all tables
+    size_t blob_bytes;
+    // staging for pdf_xfxq2_host
+    void *stage;
+    size_t stage_bytes;
+    cudaStream_t streams[3];
+    cudaEvent_t ev_done[3];
+    double setup_ms;
+};
+
+struct pdfb_alphas {
+    int device;
+    AlphasDev d;
+    void *blob;
+    void *stage;
+    size_t stage_bytes;
+    cudaStream_t streams[2];
+};
+
+// launch accounting (capi.cu)
+void pdfb_count_launch(int n);
+
+// kernels' host launchers
+int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
+                      const double *q2, double *out, long long out_stride, cudaStream_t st);
+int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out,
+                       cudaStream_t st);
+int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, int n_arrays, const int *h_off,
+                       cudaStream_t st);
+int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
+                      cudaStream_t st);
+
+#define PDFB_CUDA(call)                          \
+    do {                                         \
+        cudaError_t e_ = (call);                 \
+        if (e_ != cudaSuccess) return PDFB_ECUDA; \
+    } while (0)

@@ -1,0 +1,73 @@
+"""No-GPU checks of the boundary: the library loads, exports every symbol the header declares,
+and validates arguments before touching CUDA."""
+import ctypes
+import re
+import os
+
+import numpy as np
+import pytest
+
+from paper_2009_06635_b200 import binding as B, build, workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    build.build()
+    return B.lib()
+
+
+def test_exports_every_declared_symbol(L):
+    hdr = open(os.path.join(ROOT, "include", "pdfb200.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(pdf_\w+|alphas_\w+|pdfb_\w+)\s*\(", hdr))
+    assert {"pdf_grid_load", "pdf_xfxq2", "alphas_grid_load", "alphas_q2"} <= names
+    for n in names:
+        assert hasattr(L, n), n
+    assert set(B.EXPORTS) <= names
+
+
+def test_strerror_and_codes(L):
+    assert B.strerror(0) == "ok"
+    for c in (-1, -2, -3, -4, -5, -99):
+        assert len(B.strerror(c)) > 3
+
+
+def test_load_validates_before_cuda(L):
+    g = W.grid_config1()
+    bad_x = g.x_knots.copy(); bad_x[3] = bad_x[2]
+    with pytest.raises(B.PdfbError) as e:
+        B.pdf_grid_load(bad_x, g.q_offsets, g.q_knots, g.pids, g.values)
+    assert e.value.code == -2
+    g2 = W.grid_nnpdf_shaped()
+    bad_q = g2.q_knots.copy(); bad_q[7] *= 1.0001  # sub-grid 1 no longer starts at the threshold
+    with pytest.raises(B.PdfbError) as e:
+        B.pdf_grid_load(g2.x_knots, g2.q_offsets, bad_q, g2.pids, g2.values)
+    assert e.value.code == -2
+    with pytest.raises(B.PdfbError) as e:  # a sub-grid with one knot
+        B.pdf_grid_load(g.x_knots, np.array([0, 1, 15], np.int32), g.q_knots, g.pids, g.values)
+    assert e.value.code == -2
+    with pytest.raises(B.PdfbError) as e:
+        B.alphas_grid_load([1.0, 2.0, 1.5], [0.3, 0.2, 0.25])
+    assert e.value.code == -2
+    with pytest.raises(B.PdfbError) as e:
+        B.alphas_grid_load([1.0, 2.0, 2.0], [0.3, 0.2, 0.25])  # upper sub-grid has one node
+    assert e.value.code == -2
+
+
+def test_no_device_is_a_loud_error(L):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    g = W.grid_config1()
+    with pytest.raises(B.PdfbError) as e:
+        B.load_pdf_spec(g)
+    assert e.value.code == -4  # PDFB_ECUDA: there is no CPU fallback
+
+
+def test_null_handles_rejected(L):
+    rc = L.pdf_xfxq2(None, 1, (ctypes.c_int * 1)(21), 0, None, None, None, None)
+    assert rc == -1
+    rc = L.alphas_q2(None, 0, None, None, None)
+    assert rc == -1
