@@ -98,7 +98,7 @@ def test_config5_events_and_alphas(torch_cuda, grid2, ograph2, h2):
     dq = torch_cuda.from_numpy(q2).cuda()
     out = torch_cuda.empty_like(dq)
     B.alphas_q2(ha, dq, out)
-    torch_cuda.synchronize()
+    torch_cuda.cuda.synchronize()
     check_parity(out.cpu().numpy(), oa.q2(q2), what="alphas config5")
     B.alphas_grid_free(ha)
 
@@ -114,7 +114,7 @@ def test_alphas_edges_thresholds_and_outside(torch_cuda):
     dq = torch_cuda.from_numpy(q2).cuda()
     out = torch_cuda.empty_like(dq)
     B.alphas_q2(ha, dq, out)
-    torch_cuda.synchronize()
+    torch_cuda.cuda.synchronize()
     check_parity(out.cpu().numpy(), oa.q2(q2), what="alphas edges")
     B.alphas_grid_free(ha)
 
