@@ -52,6 +52,8 @@ def lib():
         L.pdf_grid_free.argtypes = [_vp]
         L.pdf_grid_setup_ms.restype = ctypes.c_double
         L.pdf_grid_setup_ms.argtypes = [_vp]
+        L.pdf_grid_uses_smem_path.restype = ctypes.c_int
+        L.pdf_grid_uses_smem_path.argtypes = [_vp]
         L.alphas_grid_load.restype = ctypes.c_int
         L.alphas_grid_load.argtypes = [ctypes.c_int, _dp, _dp, ctypes.c_int, ctypes.POINTER(_vp)]
         L.alphas_q2.restype = ctypes.c_int
@@ -160,6 +162,10 @@ def pdf_grid_status(g) -> int:
 
 def pdf_grid_setup_ms(g) -> float:
     return float(lib().pdf_grid_setup_ms(_vp(g)))
+
+
+def pdf_grid_uses_smem_path(g) -> bool:
+    return bool(lib().pdf_grid_uses_smem_path(_vp(g)))
 
 
 def pdf_grid_free(g):

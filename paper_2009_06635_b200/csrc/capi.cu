@@ -97,7 +97,23 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     size_t o_val = align_up(o_qrec + sizeof(IntervalRec) * nq_tot, 128);
     size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad, 128);
     size_t o_raw = align_up(o_cnt + 128, 128);
-    size_t total = o_raw + sizeof(double) * knots * n_pid;
+    // shared-memory path: flavour-group slices and the aux block
+    d.nx4 = (nx + 3) & ~3;
+    d.n_groups = (n_pid + 3) / 4;
+    d.slice_bytes = nq_tot * d.nx4 * 32;
+    d.smem_ok = (nx >= 4);
+    for (int s = 0; s < n_sub; s++) if (q_offsets[s + 1] - q_offsets[s] < 4) d.smem_ok = 0;
+    d.a_xk = 0;
+    d.a_q2k = (int)align_up(d.a_xk + sizeof(double) * nx, 16);
+    d.a_xrec = (int)align_up(d.a_q2k + sizeof(double) * nq_tot, 16);
+    d.a_qrec = d.a_xrec + (int)sizeof(IntervalRec32) * nx;
+    d.a_lutx = d.a_qrec + (int)sizeof(IntervalRec32) * nq_tot;
+    d.a_lutq = d.a_lutx + 2 * PDFB_LUT_BINS;
+    d.a_subof = d.a_lutq + 2 * PDFB_LUT_BINS;
+    d.aux_bytes = (int)align_up(d.a_subof + nq_tot, 16);
+    size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid, 128);
+    size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups, 128);
+    size_t total = o_aux + d.aux_bytes;
     char *blob = nullptr;
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
     g->blob = blob; g->blob_bytes = total;
@@ -114,9 +130,34 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         cudaEventRecord(e0, 0);
         // K1: interval records for the x knots and for each sub-grid's Q^2 knots
         int xoff[2] = {0, nx};
-        rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec), 1, xoff, 0);
+        {   // host part of the aux block: raw knots, search LUTs, sub-grid of each Q^2 knot
+            std::vector<unsigned char> aux(d.aux_bytes, 0);
+            memcpy(aux.data() + d.a_xk, x_knots, sizeof(double) * nx);
+            memcpy(aux.data() + d.a_q2k, h_q2.data(), sizeof(double) * nq_tot);
+            unsigned short *lx = (unsigned short *)(aux.data() + d.a_lutx);
+            unsigned short *lq = (unsigned short *)(aux.data() + d.a_lutq);
+            const double *U = h_z.data(), *V = h_z.data() + nx;
+            d.lutx_u0 = U[0]; d.lutx_inv_h = PDFB_LUT_BINS / (U[nx - 1] - U[0]);
+            d.lutq_v0 = V[0]; d.lutq_inv_h = PDFB_LUT_BINS / (V[nq_tot - 1] - V[0]);
+            for (int b = 0, i = 0; b < PDFB_LUT_BINS; b++) {  // largest knot at or left of the bin's left edge
+                double edge = U[0] + b * (U[nx - 1] - U[0]) / PDFB_LUT_BINS;
+                while (i + 1 <= nx - 2 && U[i + 1] <= edge) i++;
+                lx[b] = (unsigned short)i;
+            }
+            for (int b = 0, m = 0; b < PDFB_LUT_BINS; b++) {
+                double edge = V[0] + b * (V[nq_tot - 1] - V[0]) / PDFB_LUT_BINS;
+                while (m + 1 <= nq_tot - 1 && V[m + 1] <= edge) m++;
+                lq[b] = (unsigned short)m;
+            }
+            for (int s2 = 0; s2 < n_sub; s2++)
+                for (int m = q_offsets[s2]; m < q_offsets[s2 + 1]; m++) aux[d.a_subof + m] = (unsigned char)s2;
+            if (cudaMemcpy(blob + o_aux, aux.data(), d.aux_bytes, cudaMemcpyHostToDevice) != cudaSuccess) { rc = PDFB_ECUDA; break; }
+        }
+        rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec),
+                                (IntervalRec32 *)(blob + o_aux + d.a_xrec), 1, xoff, 0);
         if (rc) break;
-        rc = pdfb_setup_records((const double *)(blob + o_z) + nx, (IntervalRec *)(blob + o_qrec), n_sub, d.q_off, 0);
+        rc = pdfb_setup_records((const double *)(blob + o_z) + nx, (IntervalRec *)(blob + o_qrec),
+                                (IntervalRec32 *)(blob + o_aux + d.a_qrec), n_sub, d.q_off, 0);
         if (rc) break;
         // K1: value table re-layout, sub-grid by sub-grid
         long long src = 0;
@@ -124,6 +165,9 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
             int nq = q_offsets[s + 1] - q_offsets[s];
             rc = pdfb_setup_values((const double *)(blob + o_raw) + src,
                                    (double *)(blob + o_val) + (long long)d.v_off[s] * d.kpad, nx, nq, n_pid, d.kpad, 0);
+            if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src, (double *)(blob + o_valg),
+                                                  q_offsets[s] * d.nx4, nx, d.nx4, nq, n_pid, d.n_groups,
+                                                  (long long)d.slice_bytes / 8, 0);
             src += (long long)nx * nq * n_pid;
         }
         if (rc) break;
@@ -152,6 +196,9 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     d.qrec = (const IntervalRec *)(blob + o_qrec);
     d.val = (const double *)(blob + o_val);
     d.n_invalid = (unsigned long long *)(blob + o_cnt);
+    d.valg = (const double *)(blob + o_valg);
+    d.aux = (const unsigned char *)(blob + o_aux);
+    if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
     *out = g;
     return PDFB_OK;
 }
@@ -178,6 +225,8 @@ extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long lo
     if (rc) return rc;
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream);
 }
+
+extern "C" int pdf_grid_uses_smem_path(const pdfb_grid *g) { return g ? g->d.smem_ok : 0; }
 
 extern "C" int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points)
 {

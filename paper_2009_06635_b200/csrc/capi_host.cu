@@ -56,7 +56,7 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
         cudaMemcpy(blob + o_a, alphas, sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(blob + o_z, h_z.data(), sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess)
         rc = PDFB_ECUDA;
-    if (!rc) rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_rec), n_sub, d.off, 0);
+    if (!rc) rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_rec), nullptr, n_sub, d.off, 0);
     if (!rc && cudaDeviceSynchronize() != cudaSuccess) rc = PDFB_ECUDA;
     if (rc) { cudaFree(blob); delete a; return rc; }
     d.q2k = (const double *)(blob + o_q2);

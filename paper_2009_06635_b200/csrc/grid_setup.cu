@@ -10,13 +10,15 @@
 #include "pdfb_internal.cuh"
 
 // One thread per interval m of the knot array z[0..M-1] (natural logs of the knots).
-__global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *__restrict__ rec, int M)
+__global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *__restrict__ rec,
+                                    IntervalRec32 *__restrict__ rec32, int M)
 {
     int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= M - 1) {
         if (m == M - 1) {  // pad entry so every knot index has a record; never used by a cell
             IntervalRec r = {z[m], 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             rec[m] = r;
+            if (rec32) { IntervalRec32 q = {z[m], 0.0, 0.0, 0.0}; rec32[m] = q; }
         }
         return;
     }
@@ -37,6 +39,26 @@ __global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *_
         r.aH0 = -0.5; r.aH1 = 0.5 * (1.0 - rho); r.aHp = 0.5 * rho;
     }
     rec[m] = r;
+    if (rec32) { IntervalRec32 q = {r.z0, r.inv_dz, r.aLm, r.aHp}; rec32[m] = q; }
+}
+
+// values of one sub-grid: file order [ix][iq][ipid] -> flavour-group slices [g][iq][ix4][4]
+// (the shared-memory path stages one slice per CTA); padding columns / knots = 0
+__global__ void k1_group_slices(const double *__restrict__ src, double *__restrict__ valg, int s_knot_off,
+                                int nx, int nx4, int nq, int n_pid, int n_groups, long long group_stride)
+{
+    long long tot = (long long)n_groups * nq * nx4 * 4;
+    for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
+         e += (long long)gridDim.x * blockDim.x) {
+        int slot = (int)(e & 3);
+        long long r = e >> 2;
+        int ix = (int)(r % nx4); r /= nx4;
+        int iq = (int)(r % nq);
+        int grp = (int)(r / nq);
+        int k = grp * 4 + slot;
+        double v = (ix < nx && k < n_pid) ? src[((long long)ix * nq + iq) * n_pid + k] : 0.0;
+        valg[grp * group_stride + ((long long)(s_knot_off + iq * nx4 + ix)) * 4 + slot] = v;
+    }
 }
 
 // values of one sub-grid: file order [ix][iq][ipid] -> [iq][ix][kpad], padding columns = 0
@@ -53,12 +75,13 @@ __global__ void k1_relayout_values(const double *__restrict__ src, double *__res
     }
 }
 
-int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, int n_arrays, const int *h_off,
-                       cudaStream_t st)
+int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_rec32, int n_arrays,
+                       const int *h_off, cudaStream_t st)
 {
     for (int a = 0; a < n_arrays; a++) {
         int M = h_off[a + 1] - h_off[a];
-        k1_interval_records<<<(M + 127) / 128, 128, 0, st>>>(d_z + h_off[a], d_rec + h_off[a], M);
+        k1_interval_records<<<(M + 127) / 128, 128, 0, st>>>(d_z + h_off[a], d_rec + h_off[a],
+                                                             d_rec32 ? d_rec32 + h_off[a] : nullptr, M);
         pdfb_count_launch(1);
     }
     PDFB_CUDA(cudaGetLastError());
@@ -72,6 +95,18 @@ int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_
     int blocks = (int)((tot + 255) / 256);
     if (blocks > 1184) blocks = 1184;
     k1_relayout_values<<<blocks, 256, 0, st>>>(d_src, d_dst, nx, nq, n_pid, kpad);
+    pdfb_count_launch(1);
+    PDFB_CUDA(cudaGetLastError());
+    return PDFB_OK;
+}
+
+int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
+                            int n_pid, int n_groups, long long group_stride, cudaStream_t st)
+{
+    long long tot = (long long)n_groups * nq * nx4 * 4;
+    int blocks = (int)((tot + 255) / 256);
+    if (blocks > 1184) blocks = 1184;
+    k1_group_slices<<<blocks, 256, 0, st>>>(d_src, d_valg, s_knot_off, nx, nx4, nq, n_pid, n_groups, group_stride);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

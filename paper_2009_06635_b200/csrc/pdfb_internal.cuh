@@ -55,7 +55,22 @@ struct GridDev {
     const IntervalRec *qrec;           // [nq_tot]; entry q_off[s]+j = interval j of sub-grid s
     const double *val;                 // [s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
     unsigned long long *n_invalid;     // sticky counter
+    // ---- shared-memory path (xfxq2_smem.cu): flavour-group slices + a small aux block
+    int smem_ok;                       // 1 if the grid qualifies (nx >= 4, every sub-grid >= 4 Q knots)
+    int n_groups, nx4;                 // groups of 4 value columns; nx padded to a multiple of 4
+    int slice_bytes;                   // one group's slice: nq_tot * nx4 * 32 B
+    const double *valg;                // [group][s][iq][ix4][4]
+    const unsigned char *aux;          // aux block, copied verbatim into shared memory
+    int aux_bytes;
+    int a_xk, a_q2k, a_xrec, a_qrec, a_lutx, a_lutq, a_subof;  // byte offsets inside aux
+    double lutx_u0, lutx_inv_h, lutq_v0, lutq_inv_h;
 };
+#define PDFB_LUT_BINS 512
+
+// 32-byte interval record of the shared-memory path: the remaining coefficients follow from
+// "a derivative annihilates constants": aL1 = (aLm == 0 ? 1 : 1/2), aL0 = -(aLm + aL1),
+// aH0 = (aHp == 0 ? -1 : -1/2), aH1 = -(aH0 + aHp).
+struct __align__(16) IntervalRec32 { double z0, inv_dz, aLm, aHp; };
 
 struct AlphasDev {
     int K, n_sub;
@@ -98,8 +113,13 @@ int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long 
                       const double *q2, double *out, long long out_stride, cudaStream_t st);
 int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out,
                        cudaStream_t st);
-int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, int n_arrays, const int *h_off,
-                       cudaStream_t st);
+int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_rec32, int n_arrays,
+                       const int *h_off, cudaStream_t st);
+int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
+                            int n_pid, int n_groups, long long group_stride, cudaStream_t st);
+int pdfb_smem_eligible(const pdfb_grid *g);
+int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
+                           const double *q2, double *out, long long out_stride, cudaStream_t st);
 int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
                       cudaStream_t st);
 

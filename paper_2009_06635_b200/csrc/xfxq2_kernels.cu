@@ -162,6 +162,7 @@ int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long 
                       const double *q2, double *out, long long out_stride, cudaStream_t st)
 {
     if (n == 0) return PDFB_OK;
+    if (g->d.smem_ok) return pdfb_launch_xfxq2_smem(g, n_req, cols, n, x, q2, out, out_stride, st);
     ReqCols rc;
     rc.n = n_req;
     for (int r = 0; r < n_req; r++) rc.col[r] = cols[r];
