@@ -126,6 +126,10 @@ void alphas_grid_free(pdfb_alphas *a);
 
 const char *pdfb_strerror(int code);
 
+/* Diagnostic: out[i] = the library's coordinate logarithm of in[i] (device pointers, in > 0).
+ * Every ln of a knot or of a query coordinate goes through this one function (R-ln). */
+int pdfb_debug_ln(const double *in, double *out, long long n, void *cuda_stream);
+
 /* Kernels launched by this library since load (all handles); for bench accounting. */
 long long pdfb_launch_count(void);
 

@@ -65,6 +65,8 @@ def lib():
         L.pdfb_strerror.restype = ctypes.c_char_p
         L.pdfb_strerror.argtypes = [ctypes.c_int]
         L.pdfb_launch_count.restype = _ll
+        L.pdfb_debug_ln.restype = ctypes.c_int
+        L.pdfb_debug_ln.argtypes = [_vp, _vp, _ll, _vp]
         _lib = L
     return _lib
 
@@ -75,6 +77,11 @@ def strerror(code: int) -> str:
 
 def launch_count() -> int:
     return int(lib().pdfb_launch_count())
+
+
+def debug_ln(x, out, stream=None):
+    n = int(x.numel())
+    _check(lib().pdfb_debug_ln(_dev_ptr(x, n, "x"), _dev_ptr(out, n, "out"), n, _stream_ptr(stream)), "pdfb_debug_ln")
 
 
 def _f64(a):

@@ -39,7 +39,7 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
             }
             const IntervalRec r = rec[lo];
             double w[4];
-            weights4(r, (log(qv) - r.z0) * r.inv_dz, w);
+            weights4(r, (pdfb_ln(qv) - r.z0) * r.inv_dz, w);
             // knots lo-1 .. lo+2; absent ones have weight exactly 0, clamp their index
             int i0 = max(lo - 1, A.off[s]), i3 = min(lo + 2, hi);
             res = fma(w[3], al[i3], fma(w[2], al[lo + 1], fma(w[1], al[lo], w[0] * al[i0])));

@@ -25,9 +25,6 @@ extern "C" const char *pdfb_strerror(int code)
     }
 }
 
-// ln of a coordinate knot (reading R-ln).  Host side.
-static double knot_ln(double a) { return std::log(a); }
-
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // ------------------------------------------------------------------------------ PDF grid
@@ -69,12 +66,11 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     memcpy(g->pids, pids, sizeof(int) * n_pid);
 
     // host-side knot arrays: raw and ln
-    std::vector<double> h_q2(nq_tot), h_z(nx + nq_tot);
-    for (int i = 0; i < nx; i++) h_z[i] = knot_ln(x_knots[i]);
-    for (int j = 0; j < nq_tot; j++) {
-        h_q2[j] = q_knots[j] * q_knots[j];
-        h_z[nx + j] = knot_ln(h_q2[j]);
-    }
+    // (ln knots are computed on the device by K1 with the function the queries use, reading R-ln)
+    std::vector<double> h_q2(nq_tot + 1), h_z(nx + nq_tot + 1);
+    for (int j = 0; j < nq_tot; j++) h_q2[j] = q_knots[j] * q_knots[j];
+    h_q2[nq_tot] = 1.01 * h_q2[0];  // rule C's second probe scale rides along
+    if (!(x_knots[0] >= 1e-300) || !(h_q2[0] >= 1e-300)) return PDFB_EKNOTS;
     long long knots = 0;
     for (int s = 0; s < n_sub; s++) {
         d.q_off[s] = q_offsets[s];
@@ -85,14 +81,12 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     d.q_off[n_sub] = nq_tot;
     d.x_min = x_knots[0]; d.x_max = x_knots[nx - 1];
     d.q2_min = h_q2[0]; d.q2_max = h_q2[nq_tot - 1];
-    d.U0 = h_z[0]; d.U1 = h_z[1]; d.inv_dU01 = 1.0 / (h_z[1] - h_z[0]);
-    d.Va = h_z[nx + nq_tot - 2]; d.Vb = h_z[nx + nq_tot - 1]; d.inv_dVab = 1.0 / (d.Vb - d.Va);
 
     // one device blob: [xk | q2k | z (ln knots) | xrec | qrec | val | raw values | counter]
     size_t o_xk = 0;
     size_t o_q2k = align_up(o_xk + sizeof(double) * nx, 128);
-    size_t o_z = align_up(o_q2k + sizeof(double) * nq_tot, 128);
-    size_t o_xrec = align_up(o_z + sizeof(double) * (nx + nq_tot), 128);
+    size_t o_z = align_up(o_q2k + sizeof(double) * (nq_tot + 1), 128);
+    size_t o_xrec = align_up(o_z + sizeof(double) * (nx + nq_tot + 1), 128);
     size_t o_qrec = align_up(o_xrec + sizeof(IntervalRec) * nx, 128);
     size_t o_val = align_up(o_qrec + sizeof(IntervalRec) * nq_tot, 128);
     size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad, 128);
@@ -103,14 +97,15 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     d.slice_bytes = nq_tot * d.nx4 * 32;
     d.smem_ok = (nx >= 4);
     for (int s = 0; s < n_sub; s++) if (q_offsets[s + 1] - q_offsets[s] < 4) d.smem_ok = 0;
-    d.a_xk = 0;
-    d.a_q2k = (int)align_up(d.a_xk + sizeof(double) * nx, 16);
-    d.a_xrec = (int)align_up(d.a_q2k + sizeof(double) * nq_tot, 16);
-    d.a_qrec = d.a_xrec + (int)sizeof(IntervalRec32) * nx;
-    d.a_lutx = d.a_qrec + (int)sizeof(IntervalRec32) * nq_tot;
+    if (nq_tot >= 2048 || nx >= 32768) d.smem_ok = 0;  // LUT entry bit budget
+    d.a_xrec = 0;
+    d.a_qrec = d.a_xrec + 128 * nx;
+    d.a_xk = d.a_qrec + 128 * nq_tot;
+    d.a_q2k = d.a_xk + (int)sizeof(double) * nx;
+    d.a_lutx = d.a_q2k + (int)sizeof(double) * nq_tot;
     d.a_lutq = d.a_lutx + 2 * PDFB_LUT_BINS;
-    d.a_subof = d.a_lutq + 2 * PDFB_LUT_BINS;
-    d.aux_bytes = (int)align_up(d.a_subof + nq_tot, 16);
+    d.a_qoff = d.a_lutq + 2 * PDFB_LUT_BINS;
+    d.aux_bytes = (int)align_up(d.a_qoff + sizeof(int) * (n_sub + 1), 16);
     size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid, 128);
     size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups, 128);
     size_t total = o_aux + d.aux_bytes;
@@ -123,11 +118,17 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     do {
         if (cudaMemcpy(blob + o_xk, x_knots, sizeof(double) * nx, cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(blob + o_q2k, h_q2.data(), sizeof(double) * nq_tot, cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(blob + o_z, h_z.data(), sizeof(double) * (nx + nq_tot), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(blob + o_q2k, h_q2.data(), sizeof(double) * (nq_tot + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(blob + o_raw, values, sizeof(double) * knots * n_pid, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemset(blob + o_cnt, 0, 128) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         cudaEventRecord(e0, 0);
+        // K1: ln of the knots (and of rule C's probe scale), read back for the host-side tables
+        rc = pdfb_setup_ln((const double *)(blob + o_xk), (double *)(blob + o_z), nx, 0);
+        if (!rc) rc = pdfb_setup_ln((const double *)(blob + o_q2k), (double *)(blob + o_z) + nx, nq_tot + 1, 0);
+        if (rc) break;
+        if (cudaMemcpy(h_z.data(), blob + o_z, sizeof(double) * (nx + nq_tot + 1), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = PDFB_ECUDA; break; }
+        d.U0 = h_z[0]; d.U1 = h_z[1]; d.inv_dU01 = 1.0 / (h_z[1] - h_z[0]);
+        d.Va = h_z[nx + nq_tot - 2]; d.Vb = h_z[nx + nq_tot - 1]; d.inv_dVab = 1.0 / (d.Vb - d.Va);
         // K1: interval records for the x knots and for each sub-grid's Q^2 knots
         int xoff[2] = {0, nx};
         {   // host part of the aux block: raw knots, search LUTs, sub-grid of each Q^2 knot
@@ -139,18 +140,29 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
             const double *U = h_z.data(), *V = h_z.data() + nx;
             d.lutx_u0 = U[0]; d.lutx_inv_h = PDFB_LUT_BINS / (U[nx - 1] - U[0]);
             d.lutq_v0 = V[0]; d.lutq_inv_h = PDFB_LUT_BINS / (V[nq_tot - 1] - V[0]);
-            for (int b = 0, i = 0; b < PDFB_LUT_BINS; b++) {  // largest knot at or left of the bin's left edge
-                double edge = U[0] + b * (U[nx - 1] - U[0]) / PDFB_LUT_BINS;
-                while (i + 1 <= nx - 2 && U[i + 1] <= edge) i++;
-                lx[b] = (unsigned short)i;
+            const double hx = (U[nx - 1] - U[0]) / PDFB_LUT_BINS, hq = (V[nq_tot - 1] - V[0]) / PDFB_LUT_BINS;
+            const double mx = 1e-6 * hx, mq = 1e-6 * hq;  // safety margin around bin edges
+            for (int b = 0; b < PDFB_LUT_BINS; b++) {
+                double lo = U[0] + b * hx - mx, hi = U[0] + (b + 1) * hx + mx;
+                int i = 0, straddle = 0;
+                for (int k = 1; k <= nx - 2; k++) {
+                    if (U[k] <= lo) i = k;
+                    else if (U[k] <= hi) straddle = 1;
+                }
+                lx[b] = (unsigned short)((i << 1) | straddle);
             }
-            for (int b = 0, m = 0; b < PDFB_LUT_BINS; b++) {
-                double edge = V[0] + b * (V[nq_tot - 1] - V[0]) / PDFB_LUT_BINS;
-                while (m + 1 <= nq_tot - 1 && V[m + 1] <= edge) m++;
-                lq[b] = (unsigned short)m;
+            for (int b = 0; b < PDFB_LUT_BINS; b++) {
+                double lo = V[0] + b * hq - mq, hi = V[0] + (b + 1) * hq + mq;
+                int m = 0, straddle = 0;
+                for (int k = 1; k <= nq_tot - 1; k++) {
+                    if (V[k] <= lo) m = k;
+                    else if (V[k] <= hi) straddle = 1;
+                }
+                int sub = 0;
+                for (int s2 = 0; s2 < n_sub; s2++) if (q_offsets[s2] <= m) sub = s2;
+                lq[b] = (unsigned short)((m << 5) | (sub << 1) | straddle);
             }
-            for (int s2 = 0; s2 < n_sub; s2++)
-                for (int m = q_offsets[s2]; m < q_offsets[s2 + 1]; m++) aux[d.a_subof + m] = (unsigned char)s2;
+            memcpy(aux.data() + d.a_qoff, q_offsets, sizeof(int) * (n_sub + 1));
             if (cudaMemcpy(blob + o_aux, aux.data(), d.aux_bytes, cudaMemcpyHostToDevice) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         }
         rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec),
@@ -177,7 +189,7 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         cudaEventElapsedTime(&ms, e0, e1);
         g->setup_ms = ms;
         // rule C's second probe sits at the fixed scale 1.01 * q2_min: its v weights are constants
-        double qC = 1.01 * d.q2_min;
+        double qC = h_q2[nq_tot];
         int nq0 = q_offsets[1];
         if (!(qC < h_q2[nq0 - 1])) { rc = PDFB_EKNOTS; break; }
         int jC = 0;
@@ -185,7 +197,7 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         IntervalRec rC;
         if (cudaMemcpy(&rC, blob + o_qrec + sizeof(IntervalRec) * jC, sizeof(rC), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         d.jC = jC;
-        weights4(rC, (knot_ln(qC) - rC.z0) * rC.inv_dz, d.wvC);
+        weights4(rC, (h_z[nx + nq_tot] - rC.z0) * rC.inv_dz, d.wvC);
     } while (0);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (rc) { cudaFree(blob); delete g; return rc; }

@@ -40,7 +40,8 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
     AlphasDev &d = a->d;
     d.K = n_knots; d.n_sub = n_sub;
     std::vector<double> h_q2(n_knots), h_z(n_knots);
-    for (int k = 0; k < n_knots; k++) { h_q2[k] = q_knots[k] * q_knots[k]; h_z[k] = std::log(h_q2[k]); }
+    for (int k = 0; k < n_knots; k++) h_q2[k] = q_knots[k] * q_knots[k];
+    if (!(h_q2[0] >= 1e-300)) return PDFB_EKNOTS;
     for (int s = 0; s <= n_sub; s++) d.off[s] = off[s];
     for (int s = 0; s < n_sub; s++) d.q2_lo[s] = h_q2[off[s]];
     d.q2_min = h_q2[0]; d.q2_max = h_q2[n_knots - 1];
@@ -53,9 +54,9 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
     a->blob = blob;
     int rc = PDFB_OK;
     if (cudaMemcpy(blob + o_q2, h_q2.data(), sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(blob + o_a, alphas, sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess ||
-        cudaMemcpy(blob + o_z, h_z.data(), sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess)
+        cudaMemcpy(blob + o_a, alphas, sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess)
         rc = PDFB_ECUDA;
+    if (!rc) rc = pdfb_setup_ln((const double *)(blob + o_q2), (double *)(blob + o_z), n_knots, 0);
     if (!rc) rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_rec), nullptr, n_sub, d.off, 0);
     if (!rc && cudaDeviceSynchronize() != cudaSuccess) rc = PDFB_ECUDA;
     if (rc) { cudaFree(blob); delete a; return rc; }

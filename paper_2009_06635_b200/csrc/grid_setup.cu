@@ -9,6 +9,28 @@
 // table out for the evaluation kernel.
 #include "pdfb_internal.cuh"
 
+// natural logs of the knots, with the same function the queries use (reading R-ln)
+__global__ void k1_ln_knots(const double *__restrict__ raw, double *__restrict__ z, int n)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) z[i] = pdfb_ln(raw[i]);
+}
+
+int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st)
+{
+    k1_ln_knots<<<(n + 127) / 128, 128, 0, st>>>(d_raw, d_z, n);
+    pdfb_count_launch(1);
+    PDFB_CUDA(cudaGetLastError());
+    return PDFB_OK;
+}
+
+extern "C" int pdfb_debug_ln(const double *d_in, double *d_out, long long n, void *cuda_stream)
+{
+    if (!d_in || !d_out || n < 0 || n > 0x7fffffff) return PDFB_EINVAL;
+    if (n == 0) return PDFB_OK;
+    return pdfb_setup_ln(d_in, d_out, (int)n, (cudaStream_t)cuda_stream);
+}
+
 // One thread per interval m of the knot array z[0..M-1] (natural logs of the knots).
 __global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *__restrict__ rec,
                                     IntervalRec32 *__restrict__ rec32, int M)
@@ -18,7 +40,7 @@ __global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *_
         if (m == M - 1) {  // pad entry so every knot index has a record; never used by a cell
             IntervalRec r = {z[m], 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
             rec[m] = r;
-            if (rec32) { IntervalRec32 q = {z[m], 0.0, 0.0, 0.0}; rec32[m] = q; }
+            if (rec32) { IntervalRec32 q = {z[m], 0.0, 0.0, 0.0}; for (int k = 0; k < 4; k++) rec32[4 * m + k] = q; }
         }
         return;
     }
@@ -39,7 +61,10 @@ __global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *_
         r.aH0 = -0.5; r.aH1 = 0.5 * (1.0 - rho); r.aHp = 0.5 * rho;
     }
     rec[m] = r;
-    if (rec32) { IntervalRec32 q = {r.z0, r.inv_dz, r.aLm, r.aHp}; rec32[m] = q; }
+    if (rec32) {  // 4 copies = one 128-byte line: the 8 lanes of a quarter-warp read distinct bank groups
+        IntervalRec32 q = {r.z0, r.inv_dz, r.aLm, r.aHp};
+        for (int k = 0; k < 4; k++) rec32[4 * m + k] = q;
+    }
 }
 
 // values of one sub-grid: file order [ix][iq][ipid] -> flavour-group slices [g][iq][ix4][4]
@@ -81,7 +106,7 @@ int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_r
     for (int a = 0; a < n_arrays; a++) {
         int M = h_off[a + 1] - h_off[a];
         k1_interval_records<<<(M + 127) / 128, 128, 0, st>>>(d_z + h_off[a], d_rec + h_off[a],
-                                                             d_rec32 ? d_rec32 + h_off[a] : nullptr, M);
+                                                             d_rec32 ? d_rec32 + 4 * h_off[a] : nullptr, M);
         pdfb_count_launch(1);
     }
     PDFB_CUDA(cudaGetLastError());

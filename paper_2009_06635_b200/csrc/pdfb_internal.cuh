@@ -37,6 +37,58 @@ __host__ __device__ __forceinline__ void weights4(const IntervalRec &r, double t
     w[3] = h11 * r.aHp;
 }
 
+// ---------------------------------------------------------------------------------------------
+// ln of a positive, finite, normal double.  Classic argument reduction m in [sqrt(1/2), sqrt(2)),
+// s = f/(2+f), odd series in s (coefficients of the fdlibm/FreeBSD e_log.c minimax fit, < 1 ulp);
+// coefficients live in constant memory so that they are operands, not moves.
+static __constant__ double c_ln[10] = {
+    6.93147180369123816490e-01,  // ln2_hi
+    1.90821492927058770002e-10,  // ln2_lo
+    6.666666666666735130e-01,    // Lg1
+    3.999999999940941908e-01,    // Lg2
+    2.857142874366239149e-01,    // Lg3
+    2.222219843214978396e-01,    // Lg4
+    1.818357216161805012e-01,    // Lg5
+    1.531383769920937332e-01,    // Lg6
+    1.479819860511658591e-01,    // Lg7
+    0.0};
+
+__device__ __forceinline__ double ln_pos(double a)
+{
+    int hi = __double2hiint(a), lo = __double2loint(a);
+    int k = (hi >> 20) - 1023;
+    hi &= 0x000fffff;
+    const int i = (hi + 0x95f64) & 0x100000;  // mantissa above sqrt(2): halve it
+    k += i >> 20;
+    const double m = __hiloint2double(hi | (i ^ 0x3ff00000), lo);
+    const double f = m - 1.0;
+    const double d = 2.0 + f;
+    // s = f / d, correctly rounded in all but rare cases: reciprocal seed + Newton + residual
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(d));
+    double e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-d, r, 1.0);
+    r = fma(r, e, r);
+    double s = f * r;
+    s = fma(fma(-d, s, f), r, s);
+    const double dk = (double)k;
+    const double z = s * s, w = z * z;
+    const double t1 = w * fma(w, fma(w, c_ln[7], c_ln[5]), c_ln[3]);
+    const double t2 = z * fma(w, fma(w, fma(w, c_ln[8], c_ln[6]), c_ln[4]), c_ln[2]);
+    const double R = t2 + t1;
+    const double hfsq = 0.5 * f * f;
+    return fma(dk, c_ln[0], -((hfsq - fma(s, hfsq + R, dk * c_ln[1])) - f));
+}
+
+// ln of any positive finite double (reading R-ln: every coordinate logarithm of the library --
+// knots at load time, queries at run time -- goes through this one function, so a query that
+// sits on a knot gets t = 0 exactly)
+__device__ __forceinline__ double pdfb_ln(double a)
+{
+    return (a >= 2.2250738585072014e-308) ? ln_pos(a) : log(a);
+}
+
 struct GridDev {
     int n_sub, nx, n_pid, nq_tot;
     int kpad;                          // doubles per knot in `val` (>= n_pid)
@@ -62,10 +114,15 @@ struct GridDev {
     const double *valg;                // [group][s][iq][ix4][4]
     const unsigned char *aux;          // aux block, copied verbatim into shared memory
     int aux_bytes;
-    int a_xk, a_q2k, a_xrec, a_qrec, a_lutx, a_lutq, a_subof;  // byte offsets inside aux
+    int a_xk, a_q2k, a_xrec, a_qrec, a_lutx, a_lutq, a_qoff;  // byte offsets inside aux
     double lutx_u0, lutx_inv_h, lutq_v0, lutq_inv_h;
 };
 #define PDFB_LUT_BINS 512
+// aux block: xrec/qrec = 128-byte lines holding 4 copies of the 32-byte IntervalRec32 of an
+// interval; lutx[b] = (i << 1) | straddle, lutq[b] = (m << 5) | (s << 1) | straddle, where i / m
+// is the last knot at or left of the bin's left edge (m indexes the concatenated Q^2 knots,
+// s its sub-grid) and `straddle` says a knot lies inside the bin, so the guess must be
+// corrected by comparisons on the raw knots; qoff = the sub-grid knot offsets (ints).
 
 // 32-byte interval record of the shared-memory path: the remaining coefficients follow from
 // "a derivative annihilates constants": aL1 = (aLm == 0 ? 1 : 1/2), aL0 = -(aLm + aL1),
@@ -120,6 +177,7 @@ int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off,
 int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
                            const double *q2, double *out, long long out_stride, cudaStream_t st);
+int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st);
 int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
                       cudaStream_t st);
 

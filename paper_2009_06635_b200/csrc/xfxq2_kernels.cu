@@ -99,10 +99,10 @@ k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, con
         int i = find_interval(g.xk, g.nx, xv);
         IntervalRec r = load_rec(g.xrec + i);
         double w[4];
-        weights4(r, (log(xv) - r.z0) * r.inv_dz, w);
+        weights4(r, (pdfb_ln(xv) - r.z0) * r.inv_dz, w);
         u1 = make_set(i, g.nx, w);
     } else {
-        rA = (log(xv) - g.U0) * g.inv_dU01;
+        rA = (pdfb_ln(xv) - g.U0) * g.inv_dU01;
         u1.base = 0; u1.w[0] = 1.0; u1.w[1] = u1.w[2] = u1.w[3] = 0.0;
         u2.base = 0; u2.w[1] = 1.0; u2.w[0] = u2.w[2] = u2.w[3] = 0.0;
     }
@@ -112,7 +112,7 @@ k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, con
     double rB = 0.0;
     if (high_q) {  // probes at the last two Q^2 knots of the last sub-grid
         s = g.n_sub - 1; nq = g.q_off[s + 1] - g.q_off[s];
-        rB = (log(qv) - g.Va) * g.inv_dVab;
+        rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
         int base = max(nq - 4, 0), ia = nq - 2 - base, ib = nq - 1 - base;
         v1.base = v2.base = base;
         for (int b = 0; b < 4; b++) { v1.w[b] = (b == ia) ? 1.0 : 0.0; v2.w[b] = (b == ib) ? 1.0 : 0.0; }
@@ -126,7 +126,7 @@ k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, con
         int j = find_interval(g.q2k + g.q_off[s], nq, qv);
         IntervalRec r = load_rec(g.qrec + g.q_off[s] + j);
         double w[4];
-        weights4(r, (log(qv) - r.z0) * r.inv_dz, w);
+        weights4(r, (pdfb_ln(qv) - r.z0) * r.inv_dz, w);
         v1 = make_set(j, nq, w);
     }
     const int voff = g.v_off[s];

@@ -43,20 +43,7 @@ __device__ __forceinline__ double cont_e(double r, double yL, double yH)  // rea
     return fma(r, yH - yL, yL);
 }
 
-// window of 4 knots containing m-1..m+2 shifted into [0, M-1] (M >= 4); weights follow
-__device__ __forceinline__ int shift_set(int m, int M, double w[4])
-{
-    int base = m - 1;
-    if (base < 0) {            // m == 0: knot -1 carries weight exactly 0
-        w[0] = w[1]; w[1] = w[2]; w[2] = w[3]; w[3] = 0.0;
-        base = 0;
-    } else if (base + 3 > M - 1) {  // m == M-2: knot M carries weight exactly 0
-        w[3] = w[2]; w[2] = w[1]; w[1] = w[0]; w[0] = 0.0;
-        base = M - 4;
-    }
-    return base;
-}
-
+// the four 1-D weights of knots m-1..m+2 from the 32-byte interval record
 __device__ __forceinline__ void weights_rec32(const IntervalRec32 &r, double t, double w[4])
 {
     double t2 = t * t, t3 = t2 * t;
@@ -72,121 +59,174 @@ __device__ __forceinline__ void weights_rec32(const IntervalRec32 &r, double t, 
     w[3] = h11 * r.aHp;
 }
 
-// x-direction state of one point: smem byte offset of knot node0 within a table row, the
-// rotated chunk offsets and the x weights in rotated order
-struct USet { uint32_t off[8]; double wrot[8]; int rot; };
+// x-direction state of one point.  The 128-byte run of knots node0..node0+3 (4 columns each)
+// holds chunk c = 2*(knot - node0) + (column pair): lane l reads, at step s, chunk
+//   c(s) = ((s + rot) & 7) ^ (l & 1),   rot = ((l & 6) - 2*node0) & 7   (even),
+// which puts the 8 lanes of a quarter-warp on 8 distinct bank groups at every step.  Steps 2k and
+// 2k+1 both belong to knot slot (k + rot/2) & 3, so one rotated weight W[k] serves both; even
+// steps deliver column pair (l & 1), odd steps the other pair (resolved at the store).
+struct USet { uint32_t off[8]; double W[4]; };
 
-__device__ __forceinline__ void make_uset(USet &u, int node0, const double w[4], int lane8)
+// node0 = clamp(i-1, 0, nx-4).  A window shifted by sh = node0 - (i-1) is a cyclic rotation of
+// the weights, because the knot that wraps around carries weight exactly 0 (one-sided rule).
+__device__ __forceinline__ void make_uset(USet &u, int i, int nx, const double w[4], int lane8)
 {
-    int rot = (lane8 - 2 * node0) & 7;
-    u.rot = rot;
+    const int node0 = min(max(i - 1, 0), nx - 4);
+    const int rot = ((lane8 & 6) - 2 * node0) & 7;
+    const uint32_t nb = (uint32_t)node0 * 32u, par = (uint32_t)(lane8 & 1) << 4;
 #pragma unroll
-    for (int s = 0; s < 8; s++) u.off[s] = (uint32_t)(node0 * 32 + (((s + rot) & 7) << 4));
-    // wrot[s] = w[((s + rot) & 7) >> 1]: barrel rotation of {w0,w0,w1,w1,w2,w2,w3,w3}
-    double a[8] = {w[0], w[0], w[1], w[1], w[2], w[2], w[3], w[3]}, b[8];
+    for (int s = 0; s < 8; s++) u.off[s] = nb + ((uint32_t)(((s + rot) & 7) << 4) ^ par);
+    const int rk = ((rot >> 1) + node0 - (i - 1)) & 3;  // W[k] = w[(k + rk) & 3]
+    double a[4];
 #pragma unroll
-    for (int s = 0; s < 8; s++) b[s] = (rot & 1) ? a[(s + 1) & 7] : a[s];
+    for (int k = 0; k < 4; k++) a[k] = (rk & 1) ? w[(k + 1) & 3] : w[k];
 #pragma unroll
-    for (int s = 0; s < 8; s++) a[s] = (rot & 2) ? b[(s + 2) & 7] : b[s];
-#pragma unroll
-    for (int s = 0; s < 8; s++) u.wrot[s] = (rot & 4) ? a[(s + 4) & 7] : a[s];
+    for (int k = 0; k < 4; k++) u.W[k] = (rk & 2) ? a[(k + 2) & 3] : a[k];
 }
 
-// sum_b wv[b] * sum_a wu[a] * V[row0+b][node0+a][0..3] -> y[4]
-__device__ __forceinline__ void gather4(uint32_t tab, uint32_t row_bytes, int row0, const USet &u,
-                                        const double wv[4], double y[4])
+// rows j-1..j+2 of a sub-grid with nq >= 4 rows; a row outside wraps by 4 (its weight is exactly 0)
+struct VSet { uint32_t rowaddr[4]; double w[4]; };
+
+__device__ __forceinline__ void make_vset(VSet &v, uint32_t tab, uint32_t row_bytes, int qo, int j, int nq)
 {
-    double2 tE = make_double2(0.0, 0.0), tO = make_double2(0.0, 0.0);
-    uint32_t base = tab + (uint32_t)row0 * row_bytes;
+    const int r0 = (j == 0) ? 3 : j - 1, r3 = (j == nq - 2) ? j - 2 : j + 2;
+    v.rowaddr[0] = tab + (uint32_t)(qo + r0) * row_bytes;
+    v.rowaddr[1] = tab + (uint32_t)(qo + j) * row_bytes;
+    v.rowaddr[2] = v.rowaddr[1] + row_bytes;
+    v.rowaddr[3] = tab + (uint32_t)(qo + r3) * row_bytes;
+}
+
+// sum_b wv[b] * sum_a wu[a] * V[row_b][node0+a][cols] -> yE = column pair (lane & 1), yO = the other
+__device__ __forceinline__ void gather4(const USet &u, const VSet &v, double2 &yE, double2 &yO)
+{
+    yE = make_double2(0.0, 0.0); yO = make_double2(0.0, 0.0);
 #pragma unroll
     for (int b = 0; b < 4; b++) {
-        double2 E = make_double2(0.0, 0.0), O = make_double2(0.0, 0.0);
+        double2 c[8];
 #pragma unroll
-        for (int s = 0; s < 8; s += 2) {
-            double2 v0 = lds128(base + u.off[s]), v1 = lds128(base + u.off[s + 1]);
-            E.x = fma(u.wrot[s], v0.x, E.x); E.y = fma(u.wrot[s], v0.y, E.y);
-            O.x = fma(u.wrot[s + 1], v1.x, O.x); O.y = fma(u.wrot[s + 1], v1.y, O.y);
+        for (int s = 0; s < 8; s++) c[s] = lds128(v.rowaddr[b] + u.off[s]);
+        double2 E, O;
+        E.x = u.W[0] * c[0].x; E.y = u.W[0] * c[0].y;
+        O.x = u.W[0] * c[1].x; O.y = u.W[0] * c[1].y;
+#pragma unroll
+        for (int k = 1; k < 4; k++) {
+            E.x = fma(u.W[k], c[2 * k].x, E.x); E.y = fma(u.W[k], c[2 * k].y, E.y);
+            O.x = fma(u.W[k], c[2 * k + 1].x, O.x); O.y = fma(u.W[k], c[2 * k + 1].y, O.y);
         }
-        tE.x = fma(wv[b], E.x, tE.x); tE.y = fma(wv[b], E.y, tE.y);
-        tO.x = fma(wv[b], O.x, tO.x); tO.y = fma(wv[b], O.y, tO.y);
-        base += row_bytes;
+        yE.x = fma(v.w[b], E.x, yE.x); yE.y = fma(v.w[b], E.y, yE.y);
+        yO.x = fma(v.w[b], O.x, yO.x); yO.y = fma(v.w[b], O.y, yO.y);
     }
-    // even steps carried chunk parity (rot & 1): chunk parity 0 = columns 0,1; 1 = columns 2,3
-    bool sw = u.rot & 1;
-    y[0] = sw ? tO.x : tE.x; y[1] = sw ? tO.y : tE.y;
-    y[2] = sw ? tE.x : tO.x; y[3] = sw ? tE.y : tO.y;
 }
 
 struct SmemViews {
-    uint32_t tab, row_bytes;
+    uint32_t tab, row_bytes, xrec, qrec;  // shared-space byte addresses
     const double *xk, *q2k;
-    const IntervalRec32 *xrec, *qrec;
     const unsigned short *lutx, *lutq;
-    const unsigned char *subof;
+    const int *qoff;
 };
 
-// points outside the grid (readings O4/O5): up to 2 x-sets times 2 v-sets
-__device__ __noinline__ void slow_point(const GridDev &g, const SmemViews &sv, double xv, double qv,
-                                        int lane8, double res[4])
+// 32-byte interval record from its 128-byte line of 4 copies: lanes 2k and 2k+1 of a
+// quarter-warp use copy k and read its two 16-byte halves in opposite order, so the 8 lanes
+// touch 8 distinct bank groups at both steps whatever records they want.
+__device__ __forceinline__ IntervalRec32 load_rec4(uint32_t line, int lane8)
 {
+    const uint32_t copy = line + (uint32_t)((lane8 >> 1) << 5);
+    const uint32_t h = (uint32_t)(lane8 & 1) << 4;
+    const double2 A = lds128(copy + h), B = lds128(copy + (h ^ 16u));
+    IntervalRec32 r;
+    r.z0 = h ? B.x : A.x; r.inv_dz = h ? B.y : A.y;
+    r.aLm = h ? A.x : B.x; r.aHp = h ? A.y : B.y;
+    return r;
+}
+
+// interval of x: LUT guess, corrected by comparisons on the raw knots where a knot lies in the bin
+__device__ __forceinline__ int locate_x(const GridDev &g, const SmemViews &sv, double xv, double u)
+{
+    int b = min(max((int)((u - g.lutx_u0) * g.lutx_inv_h), 0), PDFB_LUT_BINS - 1);
+    int e = sv.lutx[b], i = e >> 1;
+    if (e & 1)
+        while (i < g.nx - 2 && sv.xk[i + 1] <= xv) ++i;
+    return i;
+}
+
+// sub-grid and interval j of Q^2 (threshold -> upper sub-grid); returns the sub-grid's first row
+__device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, double qv, double v, int &nq, int &j)
+{
+    int b = min(max((int)((v - g.lutq_v0) * g.lutq_inv_h), 0), PDFB_LUT_BINS - 1);
+    int e = sv.lutq[b], m = e >> 5, s = (e >> 1) & 15;
+    if (e & 1) {
+        while (m < g.nq_tot - 1 && sv.q2k[m + 1] <= qv) ++m;
+        while (s + 1 < g.n_sub && sv.qoff[s + 1] <= m) ++s;
+    }
+    const int qo = sv.qoff[s];
+    nq = sv.qoff[s + 1] - qo;
+    j = min(m - qo, nq - 2);
+    return qo;
+}
+
+struct Y4 { double2 E, O; };  // column pair (lane & 1) and the other pair
+
+// points outside the grid (readings O4/O5): up to 2 x-sets times 2 v-sets
+__device__ __noinline__ Y4 slow_point(const GridDev *gp, const SmemViews *svp, double xv, double qv, int lane8)
+{
+    const GridDev &g = *gp;
+    const SmemViews &sv = *svp;
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
     USet u1, u2;
     double rA = 0.0;
     if (!low_x) {
-        double u = log(xv);
-        int b = min(max((int)((u - g.lutx_u0) * g.lutx_inv_h), 0), PDFB_LUT_BINS - 1);
-        int i = sv.lutx[b];
-        while (i < g.nx - 2 && sv.xk[i + 1] <= xv) ++i;
-        while (i > 0 && sv.xk[i] > xv) --i;
-        IntervalRec32 r = sv.xrec[i];
+        const double u = ln_pos(xv);
+        const int i = locate_x(g, sv, xv, u);
+        const IntervalRec32 r = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
         double w[4];
         weights_rec32(r, (u - r.z0) * r.inv_dz, w);
-        int node0 = shift_set(i, g.nx, w);
-        make_uset(u1, node0, w, lane8);
-    } else {  // rule A: one-hot sets on knots 0 and 1
-        rA = (log(xv) - g.U0) * g.inv_dU01;
-        double e0[4] = {1.0, 0.0, 0.0, 0.0}, e1[4] = {0.0, 1.0, 0.0, 0.0};
-        make_uset(u1, 0, e0, lane8);
-        make_uset(u2, 0, e1, lane8);
+        make_uset(u1, i, g.nx, w, lane8);
+        u2 = u1;
+    } else {  // rule A: one-hot sets on knots 0 and 1 (window of interval 1: knots 0..3)
+        rA = (pdfb_ln(xv) - g.U0) * g.inv_dU01;
+        const double e0[4] = {1.0, 0.0, 0.0, 0.0}, e1[4] = {0.0, 1.0, 0.0, 0.0};
+        make_uset(u1, 1, g.nx, e0, lane8);
+        make_uset(u2, 1, g.nx, e1, lane8);
     }
-    double wv1[4], wv2[4] = {0.0, 0.0, 0.0, 0.0};
-    int row1, row2 = 0;
+    VSet v1, v2;
     double rB = 0.0;
-    if (high_q) {  // the last two Q^2 knots of the last sub-grid
-        rB = (log(qv) - g.Va) * g.inv_dVab;
-        row1 = row2 = g.nq_tot - 4;
-        wv1[0] = wv1[1] = wv1[3] = 0.0; wv1[2] = 1.0;
-        wv2[0] = wv2[1] = wv2[2] = 0.0; wv2[3] = 1.0;
+    if (high_q) {  // the last two Q^2 knots of the last sub-grid: window of its last-but-one interval
+        rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
+        const int qo = sv.qoff[g.n_sub - 1], nq = g.nq_tot - qo;
+        make_vset(v1, sv.tab, sv.row_bytes, qo, nq - 3, nq);  // rows nq-4 .. nq-1
+        v2 = v1;
+        v1.w[0] = v1.w[1] = v1.w[3] = 0.0; v1.w[2] = 1.0;
+        v2.w[0] = v2.w[1] = v2.w[2] = 0.0; v2.w[3] = 1.0;
     } else if (low_q) {  // q_min (knot 0 of sub-grid 0) and 1.01 q_min
-        row1 = 0;
-        wv1[0] = 1.0; wv1[1] = wv1[2] = wv1[3] = 0.0;
+        const int nq = sv.qoff[1];
+        make_vset(v1, sv.tab, sv.row_bytes, 0, 1, nq);  // rows 0..3
+        v1.w[0] = 1.0; v1.w[1] = v1.w[2] = v1.w[3] = 0.0;
+        make_vset(v2, sv.tab, sv.row_bytes, 0, g.jC, nq);
 #pragma unroll
-        for (int b = 0; b < 4; b++) wv2[b] = g.wvC[b];
-        row2 = shift_set(g.jC, g.q_off[1], wv2);
+        for (int b = 0; b < 4; b++) v2.w[b] = g.wvC[b];
     } else {
-        double v = log(qv);
-        int b = min(max((int)((v - g.lutq_v0) * g.lutq_inv_h), 0), PDFB_LUT_BINS - 1);
-        int m = sv.lutq[b];
-        while (m < g.nq_tot - 1 && sv.q2k[m + 1] <= qv) ++m;
-        while (m > 0 && sv.q2k[m] > qv) --m;
-        int s = sv.subof[m];
-        int nq = g.q_off[s + 1] - g.q_off[s];
-        int j = min(m - g.q_off[s], nq - 2);
-        IntervalRec32 r = sv.qrec[g.q_off[s] + j];
-        weights_rec32(r, (v - r.z0) * r.inv_dz, wv1);
-        row1 = g.q_off[s] + shift_set(j, nq, wv1);
+        const double v = ln_pos(qv);
+        int nq, j;
+        const int qo = locate_q(g, sv, qv, v, nq, j);
+        const IntervalRec32 r = load_rec4(sv.qrec + (uint32_t)(qo + j) * 128u, lane8);
+        make_vset(v1, sv.tab, sv.row_bytes, qo, j, nq);
+        weights_rec32(r, (v - r.z0) * r.inv_dz, v1.w);
+        v2 = v1;
     }
     const bool two_v = high_q || low_q;
     double y1[4], y2[4] = {0.0, 0.0, 0.0, 0.0};
-    gather4(sv.tab, sv.row_bytes, row1, u1, wv1, y1);
-    if (two_v) gather4(sv.tab, sv.row_bytes, row2, u1, wv2, y2);
+    double2 E, O;
+    gather4(u1, v1, E, O);
+    y1[0] = E.x; y1[1] = E.y; y1[2] = O.x; y1[3] = O.y;
+    if (two_v) { gather4(u1, v2, E, O); y2[0] = E.x; y2[1] = E.y; y2[2] = O.x; y2[3] = O.y; }
     if (low_x) {
-        double h1[4], h2[4];
-        gather4(sv.tab, sv.row_bytes, row1, u2, wv1, h1);
+        gather4(u2, v1, E, O);
+        const double h1[4] = {E.x, E.y, O.x, O.y};
 #pragma unroll
         for (int k = 0; k < 4; k++) y1[k] = cont_e(rA, y1[k], h1[k]);
         if (two_v) {
-            gather4(sv.tab, sv.row_bytes, row2, u2, wv2, h2);
+            gather4(u2, v2, E, O);
+            const double h2[4] = {E.x, E.y, O.x, O.y};
 #pragma unroll
             for (int k = 0; k < 4; k++) y2[k] = cont_e(rA, y2[k], h2[k]);
         }
@@ -202,17 +242,35 @@ __device__ __noinline__ void slow_point(const GridDev &g, const SmemViews &sv, d
             if (fabs(y1[k]) >= 1e-5) gamma = fmax(-2.5, (y2[k] - y1[k]) / y1[k] / 0.01);
             r = y1[k] * pow(rho, fma(gamma, rho, 1.0 - rho));
         }
-        res[k] = r;
+        y1[k] = r;
     }
+    Y4 res;
+    res.E = make_double2(y1[0], y1[1]);
+    res.O = make_double2(y1[2], y1[3]);
+    return res;
+}
+
+// output rows of this thread's E / O column pairs (-1 = column not requested)
+struct Rows { int e0, e1, o0, o1; };
+
+__device__ __forceinline__ void store4(double *__restrict__ out, long long out_stride, long long p,
+                                       const Rows &r, double2 E, double2 O)
+{
+    if (r.e0 >= 0) __stcs(out + r.e0 * out_stride + p, E.x);
+    if (r.e1 >= 0) __stcs(out + r.e1 * out_stride + p, E.y);
+    if (r.o0 >= 0) __stcs(out + r.o0 * out_stride + p, O.x);
+    if (r.o1 >= 0) __stcs(out + r.o1 * out_stride + p, O.y);
 }
 
 __global__ void __launch_bounds__(NT_SMEM, 1)
-k_xfxq2_smem(const GridDev g, const PassList pl, long long n, const double *__restrict__ x,
-             const double *__restrict__ q2, double *__restrict__ out, long long out_stride)
+k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
+             const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
+             long long out_stride)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar;
-    const int tid = threadIdx.x;
+    __shared__ uint32_t s_wlist[NT_SMEM / 32][32];  // per-warp list of out-of-grid points
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int pass = blockIdx.x % pl.n, seq = blockIdx.x / pl.n, nseq = gridDim.x / pl.n;
     if (seq >= nseq) return;
     unsigned char *s_aux = smem + g.slice_bytes;
@@ -245,69 +303,97 @@ k_xfxq2_smem(const GridDev g, const PassList pl, long long n, const double *__re
     }
     SmemViews sv;
     sv.tab = tab; sv.row_bytes = (uint32_t)g.nx4 * 32u;
+    sv.xrec = tab + (uint32_t)(g.slice_bytes + g.a_xrec);
+    sv.qrec = tab + (uint32_t)(g.slice_bytes + g.a_qrec);
     sv.xk = reinterpret_cast<const double *>(s_aux + g.a_xk);
     sv.q2k = reinterpret_cast<const double *>(s_aux + g.a_q2k);
-    sv.xrec = reinterpret_cast<const IntervalRec32 *>(s_aux + g.a_xrec);
-    sv.qrec = reinterpret_cast<const IntervalRec32 *>(s_aux + g.a_qrec);
     sv.lutx = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutx);
     sv.lutq = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutq);
-    sv.subof = s_aux + g.a_subof;
+    sv.qoff = reinterpret_cast<const int *>(s_aux + g.a_qoff);
     const int lane8 = tid & 7;
-    const int r0 = pl.row[pass][0], r1 = pl.row[pass][1], r2 = pl.row[pass][2], r3 = pl.row[pass][3];
-
-    for (long long tile = seq; tile * NT_SMEM < n; tile += nseq) {
-        const long long p = tile * NT_SMEM + tid;
-        if (p >= n) continue;
-        const double xv = __ldg(x + p), qv = __ldg(q2 + p);
-        double y[4];
-        if (xv >= g.x_min && xv <= g.x_max && qv >= g.q2_min && qv <= g.q2_max) {
-            // ---- in range: locate (LUT guess + exact comparisons), weights, one gather
-            const double u = log(xv), v = log(qv);
-            int b = min(max((int)((u - g.lutx_u0) * g.lutx_inv_h), 0), PDFB_LUT_BINS - 1);
-            int i = sv.lutx[b];
-            while (i < g.nx - 2 && sv.xk[i + 1] <= xv) ++i;
-            while (i > 0 && sv.xk[i] > xv) --i;
-            b = min(max((int)((v - g.lutq_v0) * g.lutq_inv_h), 0), PDFB_LUT_BINS - 1);
-            int m = sv.lutq[b];
-            while (m < g.nq_tot - 1 && sv.q2k[m + 1] <= qv) ++m;
-            while (m > 0 && sv.q2k[m] > qv) --m;
-            const int s = sv.subof[m];
-            const int qo = g.q_off[s], nq = g.q_off[s + 1] - qo;
-            const int j = min(m - qo, nq - 2);
-            const IntervalRec32 rx = sv.xrec[i], rq = sv.qrec[qo + j];
-            double wu[4], wv[4];
-            weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
-            weights_rec32(rq, (v - rq.z0) * rq.inv_dz, wv);
-            const int node0 = shift_set(i, g.nx, wu);
-            const int row0 = qo + shift_set(j, nq, wv);
-            USet us;
-            make_uset(us, node0, wu, lane8);
-            gather4(tab, sv.row_bytes, row0, us, wv, y);
-        } else if (!(xv > 0.0) || !(qv > 0.0) || !(xv <= g.x_max) || isinf(qv)) {
-            y[0] = y[1] = y[2] = y[3] = __longlong_as_double(0x7ff8000000000000LL);
-            if (pass == 0) atomicAdd(g.n_invalid, 1ULL);
-        } else {
-            slow_point(g, sv, xv, qv, lane8, y);
-        }
-        if (r0 >= 0) __stcs(out + r0 * out_stride + p, y[0]);
-        if (r1 >= 0) __stcs(out + r1 * out_stride + p, y[1]);
-        if (r2 >= 0) __stcs(out + r2 * out_stride + p, y[2]);
-        if (r3 >= 0) __stcs(out + r3 * out_stride + p, y[3]);
+    Rows rows;
+    {
+        const int r0 = pl.row[pass][0], r1 = pl.row[pass][1], r2 = pl.row[pass][2], r3 = pl.row[pass][3];
+        const bool odd = lane8 & 1;
+        rows.e0 = odd ? r2 : r0; rows.e1 = odd ? r3 : r1;
+        rows.o0 = odd ? r0 : r2; rows.o1 = odd ? r1 : r3;
     }
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    int wcount = 0;  // warp-uniform: entries in this warp's list
+
+    // evaluate the listed out-of-grid points of this warp with (mostly) full lanes
+    auto flush = [&](int count) {
+        __syncwarp();
+        if (lane < count) {
+            const uint32_t e = s_wlist[warp][lane];
+            const long long ps = ((long long)seq + (long long)(e >> 5) * nseq) * NT_SMEM + warp * 32 + (e & 31);
+            const Y4 r = slow_point(&g, &sv, __ldg(x + ps), __ldg(q2 + ps), lane8);
+            Rows rs = rows;  // the listed point belongs to lane (e & 31): its parity decides nothing here,
+            store4(out, out_stride, ps, rs, r.E, r.O);  // columns follow THIS lane's parity (gather is per lane)
+        }
+        __syncwarp();
+    };
+
+    // software pipeline: the next tile's coordinates are in flight while this tile is evaluated
+    long long tile = seq;
+    long long p = tile * NT_SMEM + tid;
+    double xv = (p < n) ? __ldg(x + p) : 1.0, qv = (p < n) ? __ldg(q2 + p) : 1.0;
+    for (uint32_t it = 0; tile * NT_SMEM < n; tile += nseq, ++it) {
+        p = tile * NT_SMEM + tid;
+        const long long pn = p + (long long)nseq * NT_SMEM;
+        const double xn = (pn < n) ? __ldg(x + pn) : 1.0, qn = (pn < n) ? __ldg(q2 + pn) : 1.0;
+        const bool live = p < n;
+        const bool in_range = live && xv >= g.x_min && xv <= g.x_max && qv >= g.q2_min && qv <= g.q2_max;
+        if (in_range) {
+            // ---- locate (LUT guess + exact comparisons where needed), weights, one gather
+            const double u = ln_pos(xv), v = ln_pos(qv);
+            const int i = locate_x(g, sv, xv, u);
+            int nq, j;
+            const int qo = locate_q(g, sv, qv, v, nq, j);
+            const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
+            const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)(qo + j) * 128u, lane8);
+            double wu[4];
+            USet us;
+            VSet vs;
+            weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
+            weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vs.w);
+            make_uset(us, i, g.nx, wu, lane8);
+            make_vset(vs, tab, sv.row_bytes, qo, j, nq);
+            double2 E, O;
+            gather4(us, vs, E, O);
+            store4(out, out_stride, p, rows, E, O);
+        }
+        const bool invalid = live && !in_range && (!(xv > 0.0) || !(qv > 0.0) || !(xv <= g.x_max) || isinf(qv));
+        const bool slow = live && !in_range && !invalid;
+        const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
+        if (invalid) {
+            store4(out, out_stride, p, rows, make_double2(qnan, qnan), make_double2(qnan, qnan));
+            if (pass == 0) atomicAdd(g.n_invalid, 1ULL);
+        }
+        if (slow_mask) {  // warp-uniform: compact out-of-grid points into this warp's list
+            const int k = __popc(slow_mask);
+            if (wcount + k > 32) { flush(wcount); wcount = 0; }
+            if (slow) s_wlist[warp][wcount + __popc(slow_mask & ((1u << lane) - 1u))] = (it << 5) | (uint32_t)lane;
+            wcount += k;
+        }
+        xv = xn; qv = qn;
+    }
+    if (wcount) flush(wcount);
 }
 
 static int smem_needed(const GridDev &d) { return d.slice_bytes + d.aux_bytes; }
+static const int STATIC_SMEM = 2304;  // >= the kernel's static shared memory (mbarrier, list)
 
 int pdfb_smem_eligible(const pdfb_grid *g)
 {
     if (getenv("PDFB_FORCE_FALLBACK")) return 0;  // testing: force the read-only-cache path
     int dev_max = 0;
     if (cudaDeviceGetAttribute(&dev_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, g->device) != cudaSuccess) return 0;
-    if (smem_needed(g->d) + 1024 > dev_max) return 0;
+    if (smem_needed(g->d) + STATIC_SMEM > dev_max) return 0;
     // the attribute is per function, not per handle: raise it once to the device maximum
     static int attr_set_for = -1;
     if (attr_set_for != g->device) {
-        if (cudaFuncSetAttribute(k_xfxq2_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - 1024) != cudaSuccess) {
+        if (cudaFuncSetAttribute(k_xfxq2_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - STATIC_SMEM) != cudaSuccess) {
             cudaGetLastError();
             return 0;
         }

@@ -42,6 +42,26 @@ def h2(torch_cuda, grid2):
     B.pdf_grid_free(h)
 
 
+def test_coordinate_ln_is_almost_always_correctly_rounded(torch_cuda):
+    rng = np.random.default_rng(17)
+    a = np.concatenate([np.exp(rng.uniform(np.log(1e-12), np.log(1e12), 400_000)),
+                        1.0 + rng.uniform(-0.3, 0.4, 100_000), [1.0, 2.0, 0.5, 1e-300, 1e300, 5e-324]])
+    d = torch_cuda.from_numpy(a).cuda()
+    out = torch_cuda.empty_like(d)
+    B.debug_ln(d, out)
+    got = out.cpu().numpy()
+    ref = np.array([oracle.ln(float(v)) for v in a])
+    ulp = np.abs(got - ref) / np.spacing(np.abs(ref) + 1e-300)
+    assert ulp.max() <= 1.0, ulp.max()
+    frac = float((got != ref).mean())
+    print("ln: fraction not correctly rounded", frac)
+    assert frac < 0.02
+
+
+def test_smem_path_is_the_one_that_runs(h1, h2):
+    assert B.pdf_grid_uses_smem_path(h1) and B.pdf_grid_uses_smem_path(h2)
+
+
 def test_knots_reproduced_exactly(torch_cuda, grid2, h2):
     for s in range(grid2.n_sub):
         q2 = grid2.sub_q(s) ** 2
