@@ -25,7 +25,7 @@ struct PassList {
     int row[PDFB_MAX_PIDS][4];  // output row of each of the group's 4 columns, -1 = not requested
 };
 
-#define NT_SMEM 512
+#define NT_SMEM 384
 
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
@@ -122,8 +122,22 @@ struct SmemViews {
     uint32_t tab, row_bytes, xrec, qrec;  // shared-space byte addresses
     const double *xk, *q2k;
     const unsigned short *lutx, *lutq;
-    const int *qoff;
 };
+
+__device__ __forceinline__ SmemViews make_views(const GridDev &g, unsigned char *smem)
+{
+    SmemViews sv;
+    unsigned char *s_aux = smem + g.slice_bytes;
+    sv.tab = (uint32_t)__cvta_generic_to_shared(smem);
+    sv.row_bytes = (uint32_t)g.nx4 * 32u;
+    sv.xrec = sv.tab + (uint32_t)(g.slice_bytes + g.a_xrec);
+    sv.qrec = sv.tab + (uint32_t)(g.slice_bytes + g.a_qrec);
+    sv.xk = reinterpret_cast<const double *>(s_aux + g.a_xk);
+    sv.q2k = reinterpret_cast<const double *>(s_aux + g.a_q2k);
+    sv.lutx = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutx);
+    sv.lutq = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutq);
+    return sv;
+}
 
 // 32-byte interval record from its 128-byte line of 4 copies: lanes 2k and 2k+1 of a
 // quarter-warp use copy k and read its two 16-byte halves in opposite order, so the 8 lanes
@@ -156,10 +170,10 @@ __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, d
     int e = sv.lutq[b], m = e >> 5, s = (e >> 1) & 15;
     if (e & 1) {
         while (m < g.nq_tot - 1 && sv.q2k[m + 1] <= qv) ++m;
-        while (s + 1 < g.n_sub && sv.qoff[s + 1] <= m) ++s;
+        while (s + 1 < g.n_sub && g.q_off[s + 1] <= m) ++s;
     }
-    const int qo = sv.qoff[s];
-    nq = sv.qoff[s + 1] - qo;
+    const int qo = g.q_off[s];
+    nq = g.q_off[s + 1] - qo;
     j = min(m - qo, nq - 2);
     return qo;
 }
@@ -167,10 +181,10 @@ __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, d
 struct Y4 { double2 E, O; };  // column pair (lane & 1) and the other pair
 
 // points outside the grid (readings O4/O5): up to 2 x-sets times 2 v-sets
-__device__ __noinline__ Y4 slow_point(const GridDev *gp, const SmemViews *svp, double xv, double qv, int lane8)
+__device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
 {
     const GridDev &g = *gp;
-    const SmemViews &sv = *svp;
+    const SmemViews sv = make_views(g, smem);
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
     USet u1, u2;
     double rA = 0.0;
@@ -192,13 +206,13 @@ __device__ __noinline__ Y4 slow_point(const GridDev *gp, const SmemViews *svp, d
     double rB = 0.0;
     if (high_q) {  // the last two Q^2 knots of the last sub-grid: window of its last-but-one interval
         rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
-        const int qo = sv.qoff[g.n_sub - 1], nq = g.nq_tot - qo;
+        const int qo = g.q_off[g.n_sub - 1], nq = g.nq_tot - qo;
         make_vset(v1, sv.tab, sv.row_bytes, qo, nq - 3, nq);  // rows nq-4 .. nq-1
         v2 = v1;
         v1.w[0] = v1.w[1] = v1.w[3] = 0.0; v1.w[2] = 1.0;
         v2.w[0] = v2.w[1] = v2.w[2] = 0.0; v2.w[3] = 1.0;
     } else if (low_q) {  // q_min (knot 0 of sub-grid 0) and 1.01 q_min
-        const int nq = sv.qoff[1];
+        const int nq = g.q_off[1];
         make_vset(v1, sv.tab, sv.row_bytes, 0, 1, nq);  // rows 0..3
         v1.w[0] = 1.0; v1.w[1] = v1.w[2] = v1.w[3] = 0.0;
         make_vset(v2, sv.tab, sv.row_bytes, 0, g.jC, nq);
@@ -301,15 +315,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
                          : "=r"(done) : "r"(mb) : "memory");
     }
-    SmemViews sv;
-    sv.tab = tab; sv.row_bytes = (uint32_t)g.nx4 * 32u;
-    sv.xrec = tab + (uint32_t)(g.slice_bytes + g.a_xrec);
-    sv.qrec = tab + (uint32_t)(g.slice_bytes + g.a_qrec);
-    sv.xk = reinterpret_cast<const double *>(s_aux + g.a_xk);
-    sv.q2k = reinterpret_cast<const double *>(s_aux + g.a_q2k);
-    sv.lutx = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutx);
-    sv.lutq = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutq);
-    sv.qoff = reinterpret_cast<const int *>(s_aux + g.a_qoff);
+    const SmemViews sv = make_views(g, smem);
     const int lane8 = tid & 7;
     Rows rows;
     {
@@ -327,7 +333,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         if (lane < count) {
             const uint32_t e = s_wlist[warp][lane];
             const long long ps = ((long long)seq + (long long)(e >> 5) * nseq) * NT_SMEM + warp * 32 + (e & 31);
-            const Y4 r = slow_point(&g, &sv, __ldg(x + ps), __ldg(q2 + ps), lane8);
+            const Y4 r = slow_point(&g, smem, __ldg(x + ps), __ldg(q2 + ps), lane8);
             Rows rs = rows;  // the listed point belongs to lane (e & 31): its parity decides nothing here,
             store4(out, out_stride, ps, rs, r.E, r.O);  // columns follow THIS lane's parity (gather is per lane)
         }
