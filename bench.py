@@ -27,6 +27,9 @@ from paper_2009_06635_b200 import workloads as W  # noqa: E402
 METRIC = "pdf_evaluations_per_sec"
 UNIT = "evaluations/s"
 N_FULL = 100_000_000
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_xfxq2_smem launch at 1e8 points x 11
+# flavours, from the `ncu --set full` capture summarised in profiles/r1_xfxq2_smem_full.md
+NCU_TRAFFIC_BYTES_PER_POINT = (1.641881e9 + 8.743990e9) / 1e8
 
 
 def measured_peaks():
@@ -231,7 +234,9 @@ def run_gpu(args):
                        "grid_setup_ms": B.pdf_grid_setup_ms(h)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": "k_xfxq2", "kernel_ms": kern_ms,
+                         "traffic": (NCU_TRAFFIC_BYTES_PER_POINT * n / 1e9) if F == 11 else None, "traffic_unit": "GB per launch",
+                         "traffic_source": "profiles/r1_xfxq2_smem_full.md (ncu, 1e8 points; scaled by points)",
+                         "kernel": "k_xfxq2_smem" if B.pdf_grid_uses_smem_path(h) else "k_xfxq2_v0", "kernel_ms": kern_ms,
                          "algorithmic_bytes_per_point": 16 + 8 * F, "peak_source": peak_src},
             "alphas": {"points": n, "ms": a_ms, "evaluations_per_s": n / (a_ms * 1e-3),
                        "hbm_frac": 16 * n / (a_ms * 1e-3) / 1e9 / peak}}
