@@ -48,9 +48,74 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
     }
 }
 
+// Fast path (K <= 192 nodes): replicated coefficient lines in shared memory, LUT location,
+// one cubic in t per point.  Two points per thread keep two independent ln chains in flight.
+#define NT_ALPHAS 512
+
+__global__ void __launch_bounds__(NT_ALPHAS, 2)
+k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__restrict__ q2,
+              double *__restrict__ out)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    for (int e = threadIdx.x; e < A.fast_bytes / 16; e += NT_ALPHAS)
+        reinterpret_cast<int4 *>(smem)[e] = __ldg(reinterpret_cast<const int4 *>(A.fast) + e);
+    __syncthreads();
+    const uint32_t lines = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)((threadIdx.x & 7) << 4);
+    const double *q2k = reinterpret_cast<const double *>(smem + A.f_q2k);
+    const unsigned short *lut = reinterpret_cast<const unsigned short *>(smem + A.f_lut);
+    const double qnan = __longlong_as_double(0x7ff8000000000000LL);
+    auto eval = [&](double qv) -> double {
+        double res;
+        if (qv >= A.q2_min && qv <= A.q2_max) {
+            const double v = pdfb_ln(qv);
+            int b = min(max((int)((v - A.lut_v0) * A.lut_inv_h), 0), PDFB_LUT_BINS - 1);
+            int e = lut[b], m = e >> 1;
+            if (e & 1)
+                while (m < A.K - 1 && q2k[m + 1] <= qv) ++m;
+            m = min(m, A.K - 2);  // Q^2 = last node: last interval, t = 1
+            const uint32_t rec = lines + (uint32_t)m * 512u;
+            double2 zi, c01, c23;
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(zi.x), "=d"(zi.y) : "r"(rec));
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(c01.x), "=d"(c01.y) : "r"(rec + 128u));
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(c23.x), "=d"(c23.y) : "r"(rec + 256u));
+            const double t = (v - zi.x) * zi.y;
+            res = fma(t, fma(t, fma(t, c23.y, c23.x), c01.y), c01.x);
+        } else {
+            res = (qv < A.q2_min) ? A.a_first : A.a_last;
+        }
+        return (qv > 0.0) ? res : qnan;  // NaN and non-positive Q^2 have no value
+    };
+    // 4 points per thread and iteration: the loads go out together, the ln chains interleave
+    const long long stride = (long long)gridDim.x * NT_ALPHAS;
+    long long p = blockIdx.x * (long long)NT_ALPHAS + threadIdx.x;
+    for (; p + 3 * stride < n; p += 4 * stride) {
+        double q[4], r[4];
+#pragma unroll
+        for (int k = 0; k < 4; k++) q[k] = __ldcs(q2 + p + k * stride);
+#pragma unroll
+        for (int k = 0; k < 4; k++) r[k] = eval(q[k]);
+#pragma unroll
+        for (int k = 0; k < 4; k++) __stcs(out + p + k * stride, r[k]);
+    }
+    for (; p < n; p += stride) __stcs(out + p, eval(__ldcs(q2 + p)));
+}
+
 int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out, cudaStream_t st)
 {
     if (n == 0) return PDFB_OK;
+    if (a->d.fast_ok) {
+        static int attr_dev = -1;
+        if (attr_dev != a->device) {
+            PDFB_CUDA(cudaFuncSetAttribute(k_alphas_fast, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
+            attr_dev = a->device;
+        }
+        long long blocks = (n + NT_ALPHAS - 1) / NT_ALPHAS;
+        if (blocks > 148 * 2) blocks = 148 * 2;
+        k_alphas_fast<<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
+        pdfb_count_launch(1);
+        PDFB_CUDA(cudaGetLastError());
+        return PDFB_OK;
+    }
     size_t smem = (size_t)a->d.K * (sizeof(IntervalRec) + 16);
     long long blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;

@@ -48,7 +48,13 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
     d.a_first = alphas[0]; d.a_last = alphas[n_knots - 1];
 
     size_t o_q2 = 0, o_a = align_up(sizeof(double) * n_knots, 128), o_z = 2 * o_a, o_rec = 3 * o_a;
-    size_t total = o_rec + sizeof(IntervalRec) * n_knots;
+    // fast-path block: [lines K*512][q2k K doubles][lut u16]
+    d.fast_ok = (n_knots <= 192);
+    d.f_q2k = 512 * n_knots;
+    d.f_lut = d.f_q2k + (int)sizeof(double) * n_knots;
+    d.fast_bytes = (int)align_up(d.f_lut + 2 * PDFB_LUT_BINS, 16);
+    size_t o_fast = align_up(o_rec + sizeof(IntervalRec) * n_knots, 128);
+    size_t total = o_fast + d.fast_bytes;
     char *blob = nullptr;
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete a; return PDFB_ECUDA; }
     a->blob = blob;
@@ -58,8 +64,29 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
         rc = PDFB_ECUDA;
     if (!rc) rc = pdfb_setup_ln((const double *)(blob + o_q2), (double *)(blob + o_z), n_knots, 0);
     if (!rc) rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_rec), nullptr, n_sub, d.off, 0);
+    if (!rc) rc = pdfb_setup_alphas_fast((const IntervalRec *)(blob + o_rec), (const double *)(blob + o_a),
+                                         (unsigned char *)(blob + o_fast), n_sub, d.off, 0);
+    if (!rc && cudaMemcpy(h_z.data(), blob + o_z, sizeof(double) * n_knots, cudaMemcpyDeviceToHost) != cudaSuccess) rc = PDFB_ECUDA;
+    if (!rc) {  // LUT over ln Q^2: (m << 1) | straddle, m = last node at or left of the bin's left edge
+        std::vector<unsigned short> lut(PDFB_LUT_BINS);
+        const double h = (h_z[n_knots - 1] - h_z[0]) / PDFB_LUT_BINS, mg = 1e-6 * h;
+        d.lut_v0 = h_z[0]; d.lut_inv_h = PDFB_LUT_BINS / (h_z[n_knots - 1] - h_z[0]);
+        for (int b = 0; b < PDFB_LUT_BINS; b++) {
+            double lo = h_z[0] + b * h - mg, hi = h_z[0] + (b + 1) * h + mg;
+            int m = 0, straddle = 0;
+            for (int k = 1; k <= n_knots - 1; k++) {
+                if (h_z[k] <= lo) m = k;
+                else if (h_z[k] <= hi) straddle = 1;
+            }
+            lut[b] = (unsigned short)((m << 1) | straddle);
+        }
+        if (cudaMemcpy(blob + o_fast + d.f_q2k, h_q2.data(), sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(blob + o_fast + d.f_lut, lut.data(), 2 * PDFB_LUT_BINS, cudaMemcpyHostToDevice) != cudaSuccess)
+            rc = PDFB_ECUDA;
+    }
     if (!rc && cudaDeviceSynchronize() != cudaSuccess) rc = PDFB_ECUDA;
     if (rc) { cudaFree(blob); delete a; return rc; }
+    d.fast = (const unsigned char *)(blob + o_fast);
     d.q2k = (const double *)(blob + o_q2);
     d.a = (const double *)(blob + o_a);
     d.rec = (const IntervalRec *)(blob + o_rec);

@@ -137,6 +137,13 @@ struct AlphasDev {
     const double *q2k;        // [K]
     const double *a;          // [K]
     const IntervalRec *rec;   // [K]
+    // fast path (alphas_kernels.cu): per interval 4 lines of 128 B; line k = the 16-byte chunk k of
+    // {ln knot, 1/d | c0, c1 | c2, c3 | pad} repeated 8 times, so lane l reads slot (l & 7) of each
+    // line: conflict-free whatever intervals the lanes want.  alpha_s(t) = c0 + t(c1 + t(c2 + t c3)).
+    int fast_ok;
+    const unsigned char *fast;  // [lines: K*512 B][q2k: K doubles][lut: PDFB_LUT_BINS u16]
+    int fast_bytes, f_q2k, f_lut;
+    double lut_v0, lut_inv_h;
 };
 
 struct pdfb_grid {
@@ -178,6 +185,8 @@ int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
                            const double *q2, double *out, long long out_stride, cudaStream_t st);
 int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st);
+int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, unsigned char *d_lines, int n_sub,
+                            const int *h_off, cudaStream_t st);
 int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
                       cudaStream_t st);
 
