@@ -198,6 +198,12 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         if (cudaMemcpy(&rC, blob + o_qrec + sizeof(IntervalRec) * jC, sizeof(rC), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         d.jC = jC;
         weights4(rC, (h_z[nx + nq_tot] - rC.z0) * rC.inv_dz, d.wvC);
+        // window form for the shared-memory path: 4 consecutive rows inside sub-grid 0; in an edge
+        // interval the window is shifted by one and the weights rotate (the wrapped weight is 0)
+        int shC = (jC == 0 ? 1 : 0) - (jC == nq0 - 2 ? 1 : 0);
+        if (nq0 < 4) shC = 0;  // such grids never take the shared-memory path
+        d.rowC = jC - 1 + shC;
+        for (int b = 0; b < 4; b++) d.wvCw[b] = d.wvC[(b + shC + 4) & 3];
     } while (0);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (rc) { cudaFree(blob); delete g; return rc; }

@@ -100,7 +100,9 @@ struct GridDev {
     double U0, U1, inv_dU01;           // ln x_0, ln x_1, 1/(U1-U0)
     double Va, Vb, inv_dVab;           // ln of the last two Q^2 knots, 1/(Vb-Va)
     int jC;                            // interval of 1.01*q2_min in sub-grid 0
-    double wvC[4];                     // its four v weights (fixed per grid)
+    double wvC[4];                     // its four v weights (fixed per grid), stencil order j-1..j+2
+    int rowC;                          // first row of its 4-row window inside sub-grid 0 (smem path)
+    double wvCw[4];                    // the same weights in window order
     const double *xk;                  // [nx] x knots
     const double *q2k;                 // [nq_tot] Q^2 knots
     const IntervalRec *xrec;           // [nx-1]

@@ -5,13 +5,20 @@
 // traffic -- and the points of a warp almost never share a cell.  The gather is what bounds the
 // kernel, so it is fed from shared memory at full crossbar width, with no bank conflict:
 //   * the value table is split into FLAVOUR GROUPS of 4 columns; one group's slice
-//     [s][iq][ix4][4] (32 B per knot) fits shared memory and is staged once per CTA by TMA bulk
-//     copies.  Each persistent CTA serves one group for all points of its tiles, so it writes
-//     whole flavour rows with coalesced stores and no point ever has to be re-ordered;
-//   * one stencil row (4 knots x 4 flavours) is 128 contiguous bytes = 8 chunks of 16 B that
+//     [iq][ix4][4] (32 B per knot, iq over the concatenated Q^2 knots) fits shared memory and is
+//     staged once per CTA by TMA bulk copies.  Each persistent CTA serves one group for all
+//     points of its tiles, so it writes whole flavour rows with coalesced stores and no point
+//     ever has to be re-ordered;
+//   * the 4x4 stencil is always read as a WINDOW of 4 consecutive rows x 4 consecutive knots that
+//     lies inside the knot array / the sub-grid: in an edge interval the window is shifted by one
+//     and the weights are rotated cyclically, which is exact because the knot that wraps around
+//     carries weight exactly 0 (one-sided derivative rule, reading O2).  Rows of a window are a
+//     uniform stride apart, so the 32 loads of a point use 8 per-lane addresses + 3 uniform
+//     offsets (LDS [R+UR]) and no address arithmetic;
+//   * one window row (4 knots x 4 flavours) is 128 contiguous bytes = 8 chunks of 16 B that
 //     cover all 8 bank groups.  Lane l reads them in the rotated order c = (s + l - 2*node0) & 7,
 //     so at every step the 8 lanes of a quarter-warp hit 8 distinct bank groups whatever cells
-//     their points fell in: 32 conflict-free LDS.128 per point and group, 4 wavefronts;
+//     their points fell in: 32 conflict-free LDS.128 per point and group, 4 wavefronts each;
 //   * the x weights are rotated the same way (selects on the ALU pipe), so no data is moved back.
 // Knot location uses a uniform-in-log lookup table corrected by comparisons on the raw knots
 // (the result is defined by the comparisons, reading Q5).
@@ -25,7 +32,9 @@ struct PassList {
     int row[PDFB_MAX_PIDS][4];  // output row of each of the group's 4 columns, -1 = not requested
 };
 
-#define NT_SMEM 384
+#ifndef NT_SMEM
+#define NT_SMEM 512
+#endif
 
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
@@ -43,68 +52,68 @@ __device__ __forceinline__ double cont_e(double r, double yL, double yH)  // rea
     return fma(r, yH - yL, yL);
 }
 
-// the four 1-D weights of knots m-1..m+2 from the 32-byte interval record
-__device__ __forceinline__ void weights_rec32(const IntervalRec32 &r, double t, double w[4])
+// The four 1-D weights of knots m-1..m+2 (stencil order) from the 32-byte interval record, and
+// the window shift sh: the window starts at knot m-1+sh, sh = +1 in the first interval of the
+// array (aLm == 0: knot m-1 does not exist), -1 in the last (aHp == 0), else 0.
+__device__ __forceinline__ int weights_sh(const IntervalRec32 &r, double t, double w[4])
 {
+    const bool first = (r.aLm == 0.0), last = (r.aHp == 0.0);
     double t2 = t * t, t3 = t2 * t;
     double h01 = 3.0 * t2 - 2.0 * t3;
     double h00 = 1.0 - h01;
     double h11 = t3 - t2;
     double h10 = h11 - t2 + t;
-    double aL1 = (r.aLm == 0.0) ? 1.0 : 0.5, aH0 = (r.aHp == 0.0) ? -1.0 : -0.5;
+    double aL1 = first ? 1.0 : 0.5, aH0 = last ? -1.0 : -0.5;
     double aL0 = -(r.aLm + aL1), aH1 = -(aH0 + r.aHp);
     w[0] = h10 * r.aLm;
     w[1] = fma(h11, aH0, fma(h10, aL0, h00));
     w[2] = fma(h11, aH1, fma(h10, aL1, h01));
     w[3] = h11 * r.aHp;
+    return (first ? 1 : 0) - (last ? 1 : 0);
 }
 
-// x-direction state of one point.  The 128-byte run of knots node0..node0+3 (4 columns each)
-// holds chunk c = 2*(knot - node0) + (column pair): lane l reads, at step s, chunk
-//   c(s) = ((s + rot) & 7) ^ (l & 1),   rot = ((l & 6) - 2*node0) & 7   (even),
-// which puts the 8 lanes of a quarter-warp on 8 distinct bank groups at every step.  Steps 2k and
-// 2k+1 both belong to knot slot (k + rot/2) & 3, so one rotated weight W[k] serves both; even
-// steps deliver column pair (l & 1), odd steps the other pair (resolved at the store).
-struct USet { uint32_t off[8]; double W[4]; };
-
-// node0 = clamp(i-1, 0, nx-4).  A window shifted by sh = node0 - (i-1) is a cyclic rotation of
-// the weights, because the knot that wraps around carries weight exactly 0 (one-sided rule).
-__device__ __forceinline__ void make_uset(USet &u, int i, int nx, const double w[4], int lane8)
+// o[k] = w[(k + r) & 3]
+__device__ __forceinline__ void rot4(const double w[4], int r, double o[4])
 {
-    const int node0 = min(max(i - 1, 0), nx - 4);
-    const int rot = ((lane8 & 6) - 2 * node0) & 7;
-    const uint32_t nb = (uint32_t)node0 * 32u, par = (uint32_t)(lane8 & 1) << 4;
-#pragma unroll
-    for (int s = 0; s < 8; s++) u.off[s] = nb + ((uint32_t)(((s + rot) & 7) << 4) ^ par);
-    const int rk = ((rot >> 1) + node0 - (i - 1)) & 3;  // W[k] = w[(k + rk) & 3]
     double a[4];
 #pragma unroll
-    for (int k = 0; k < 4; k++) a[k] = (rk & 1) ? w[(k + 1) & 3] : w[k];
+    for (int k = 0; k < 4; k++) a[k] = (r & 1) ? w[(k + 1) & 3] : w[k];
 #pragma unroll
-    for (int k = 0; k < 4; k++) u.W[k] = (rk & 2) ? a[(k + 2) & 3] : a[k];
+    for (int k = 0; k < 4; k++) o[k] = (r & 2) ? a[(k + 2) & 3] : a[k];
 }
 
-// rows j-1..j+2 of a sub-grid with nq >= 4 rows; a row outside wraps by 4 (its weight is exactly 0)
-struct VSet { uint32_t rowaddr[4]; double w[4]; };
+// One (x window, row window) pair of a point.  The 128-byte run of window knots node0..node0+3
+// (4 columns each) holds chunk c = 2*(knot - node0) + (column pair).  Lane l reads, at step s,
+//   c(s) = ((s + rot) & 7) ^ (l & 1),   rot = ((l & 6) - 2*node0) & 7   (even),
+// which puts the 8 lanes of a quarter-warp on 8 distinct bank groups at every step.  Steps 2k and
+// 2k+1 both belong to window knot (k + rot/2) & 3, so one rotated weight W[k] serves both; even
+// steps deliver column pair (l & 1), odd steps the other pair (swapped back before the store).
+struct Win { uint32_t a[8]; double W[4]; };
 
-__device__ __forceinline__ void make_vset(VSet &v, uint32_t tab, uint32_t row_bytes, int qo, int j, int nq)
+// row0 = shared address of window row 0; wu = x weights in stencil order, shx their window shift
+__device__ __forceinline__ void make_win(Win &u, uint32_t row0, int node0, int shx, const double wu[4], int lane8)
 {
-    const int r0 = (j == 0) ? 3 : j - 1, r3 = (j == nq - 2) ? j - 2 : j + 2;
-    v.rowaddr[0] = tab + (uint32_t)(qo + r0) * row_bytes;
-    v.rowaddr[1] = tab + (uint32_t)(qo + j) * row_bytes;
-    v.rowaddr[2] = v.rowaddr[1] + row_bytes;
-    v.rowaddr[3] = tab + (uint32_t)(qo + r3) * row_bytes;
+    const int rot2 = ((lane8 >> 1) - node0) & 3;
+    const uint32_t base = row0 + (uint32_t)node0 * 32u + ((uint32_t)(lane8 & 1) << 4);
+#pragma unroll
+    for (int k = 0; k < 4; k++) {
+        u.a[2 * k] = base + ((uint32_t)((k + rot2) & 3) << 5);
+        u.a[2 * k + 1] = u.a[2 * k] ^ 16u;
+    }
+    rot4(wu, (rot2 + shx) & 3, u.W);
 }
 
-// sum_b wv[b] * sum_a wu[a] * V[row_b][node0+a][cols] -> yE = column pair (lane & 1), yO = the other
-__device__ __forceinline__ void gather4(const USet &u, const VSet &v, double2 &yE, double2 &yO)
+// sum_b vw[b] * sum_k W[k] * V[window row b][window knot][cols] -> E = column pair (lane & 1), O = the other
+__device__ __forceinline__ void gather4(const Win &u, const double vw[4], uint32_t rb1, uint32_t rb2, uint32_t rb3,
+                                        double2 &yE, double2 &yO)
 {
     yE = make_double2(0.0, 0.0); yO = make_double2(0.0, 0.0);
 #pragma unroll
     for (int b = 0; b < 4; b++) {
+        const uint32_t ro = (b == 0) ? 0u : (b == 1) ? rb1 : (b == 2) ? rb2 : rb3;
         double2 c[8];
 #pragma unroll
-        for (int s = 0; s < 8; s++) c[s] = lds128(v.rowaddr[b] + u.off[s]);
+        for (int s = 0; s < 8; s++) c[s] = lds128(u.a[s] + ro);
         double2 E, O;
         E.x = u.W[0] * c[0].x; E.y = u.W[0] * c[0].y;
         O.x = u.W[0] * c[1].x; O.y = u.W[0] * c[1].y;
@@ -113,8 +122,8 @@ __device__ __forceinline__ void gather4(const USet &u, const VSet &v, double2 &y
             E.x = fma(u.W[k], c[2 * k].x, E.x); E.y = fma(u.W[k], c[2 * k].y, E.y);
             O.x = fma(u.W[k], c[2 * k + 1].x, O.x); O.y = fma(u.W[k], c[2 * k + 1].y, O.y);
         }
-        yE.x = fma(v.w[b], E.x, yE.x); yE.y = fma(v.w[b], E.y, yE.y);
-        yO.x = fma(v.w[b], O.x, yO.x); yO.y = fma(v.w[b], O.y, yO.y);
+        yE.x = fma(vw[b], E.x, yE.x); yE.y = fma(vw[b], E.y, yE.y);
+        yO.x = fma(vw[b], O.x, yO.x); yO.y = fma(vw[b], O.y, yO.y);
     }
 }
 
@@ -163,83 +172,86 @@ __device__ __forceinline__ int locate_x(const GridDev &g, const SmemViews &sv, d
     return i;
 }
 
-// sub-grid and interval j of Q^2 (threshold -> upper sub-grid); returns the sub-grid's first row
-__device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, double qv, double v, int &nq, int &j)
+// Interval of Q^2 as an index into the CONCATENATED knot list: m = the last knot <= Q^2.  A
+// threshold is stored twice (last knot of the lower sub-grid, first of the upper), so a point on
+// it lands on the upper copy (reading Q2) and the lower copy is never an interval start; only
+// Q^2 = q2_max needs the clamp.  Interval records and table rows use the same index.
+__device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, double qv, double v)
 {
     int b = min(max((int)((v - g.lutq_v0) * g.lutq_inv_h), 0), PDFB_LUT_BINS - 1);
-    int e = sv.lutq[b], m = e >> 5, s = (e >> 1) & 15;
-    if (e & 1) {
+    int e = sv.lutq[b], m = e >> 5;
+    if (e & 1)
         while (m < g.nq_tot - 1 && sv.q2k[m + 1] <= qv) ++m;
-        while (s + 1 < g.n_sub && g.q_off[s + 1] <= m) ++s;
-    }
-    const int qo = g.q_off[s];
-    nq = g.q_off[s + 1] - qo;
-    j = min(m - qo, nq - 2);
-    return qo;
+    return min(m, g.nq_tot - 2);
 }
 
 struct Y4 { double2 E, O; };  // column pair (lane & 1) and the other pair
 
-// points outside the grid (readings O4/O5): up to 2 x-sets times 2 v-sets
+// points outside the grid (readings O4/O5): up to 2 x-sets times 2 row windows
 __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
 {
     const GridDev &g = *gp;
     const SmemViews sv = make_views(g, smem);
+    const uint32_t RB = sv.row_bytes;
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
-    USet u1, u2;
+    // ---- x: one weight set in range, else the two one-hot sets of knots 0 and 1 (rule A)
+    double wu1[4] = {1.0, 0.0, 0.0, 0.0}, wu2[4] = {0.0, 1.0, 0.0, 0.0};  // window knots 0..3, shift 0
+    int node0 = 0, shx = 0;
     double rA = 0.0;
     if (!low_x) {
         const double u = ln_pos(xv);
         const int i = locate_x(g, sv, xv, u);
         const IntervalRec32 r = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
-        double w[4];
-        weights_rec32(r, (u - r.z0) * r.inv_dz, w);
-        make_uset(u1, i, g.nx, w, lane8);
-        u2 = u1;
-    } else {  // rule A: one-hot sets on knots 0 and 1 (window of interval 1: knots 0..3)
+        shx = weights_sh(r, (u - r.z0) * r.inv_dz, wu1);
+        node0 = i - 1 + shx;
+    } else {
         rA = (pdfb_ln(xv) - g.U0) * g.inv_dU01;
-        const double e0[4] = {1.0, 0.0, 0.0, 0.0}, e1[4] = {0.0, 1.0, 0.0, 0.0};
-        make_uset(u1, 1, g.nx, e0, lane8);
-        make_uset(u2, 1, g.nx, e1, lane8);
     }
-    VSet v1, v2;
+    // ---- rows: one window in range, else two probes (rules B, C)
+    int row1, row2;
+    double vw1[4], vw2[4];
     double rB = 0.0;
-    if (high_q) {  // the last two Q^2 knots of the last sub-grid: window of its last-but-one interval
+    if (high_q) {  // the last two Q^2 knots of the last sub-grid: rows 2 and 3 of its last window
         rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
-        const int qo = g.q_off[g.n_sub - 1], nq = g.nq_tot - qo;
-        make_vset(v1, sv.tab, sv.row_bytes, qo, nq - 3, nq);  // rows nq-4 .. nq-1
-        v2 = v1;
-        v1.w[0] = v1.w[1] = v1.w[3] = 0.0; v1.w[2] = 1.0;
-        v2.w[0] = v2.w[1] = v2.w[2] = 0.0; v2.w[3] = 1.0;
-    } else if (low_q) {  // q_min (knot 0 of sub-grid 0) and 1.01 q_min
-        const int nq = g.q_off[1];
-        make_vset(v1, sv.tab, sv.row_bytes, 0, 1, nq);  // rows 0..3
-        v1.w[0] = 1.0; v1.w[1] = v1.w[2] = v1.w[3] = 0.0;
-        make_vset(v2, sv.tab, sv.row_bytes, 0, g.jC, nq);
+        row1 = row2 = g.nq_tot - 4;
+        vw1[0] = vw1[1] = vw1[3] = 0.0; vw1[2] = 1.0;
+        vw2[0] = vw2[1] = vw2[2] = 0.0; vw2[3] = 1.0;
+    } else if (low_q) {  // q_min (row 0 of sub-grid 0) and 1.01 q_min (fixed window and weights)
+        row1 = 0;
+        vw1[0] = 1.0; vw1[1] = vw1[2] = vw1[3] = 0.0;
+        row2 = g.rowC;
 #pragma unroll
-        for (int b = 0; b < 4; b++) v2.w[b] = g.wvC[b];
+        for (int b = 0; b < 4; b++) vw2[b] = g.wvCw[b];
     } else {
         const double v = ln_pos(qv);
-        int nq, j;
-        const int qo = locate_q(g, sv, qv, v, nq, j);
-        const IntervalRec32 r = load_rec4(sv.qrec + (uint32_t)(qo + j) * 128u, lane8);
-        make_vset(v1, sv.tab, sv.row_bytes, qo, j, nq);
-        weights_rec32(r, (v - r.z0) * r.inv_dz, v1.w);
-        v2 = v1;
+        const int gi = locate_q(g, sv, qv, v);
+        const IntervalRec32 r = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
+        double wv[4];
+        const int shq = weights_sh(r, (v - r.z0) * r.inv_dz, wv);
+        rot4(wv, shq & 3, vw1);
+        row1 = row2 = gi - 1 + shq;
     }
     const bool two_v = high_q || low_q;
     double y1[4], y2[4] = {0.0, 0.0, 0.0, 0.0};
     double2 E, O;
-    gather4(u1, v1, E, O);
+    Win w;
+    make_win(w, sv.tab + (uint32_t)row1 * RB, node0, shx, wu1, lane8);
+    gather4(w, vw1, RB, 2 * RB, 3 * RB, E, O);
     y1[0] = E.x; y1[1] = E.y; y1[2] = O.x; y1[3] = O.y;
-    if (two_v) { gather4(u1, v2, E, O); y2[0] = E.x; y2[1] = E.y; y2[2] = O.x; y2[3] = O.y; }
+    if (two_v) {
+        make_win(w, sv.tab + (uint32_t)row2 * RB, node0, shx, wu1, lane8);
+        gather4(w, vw2, RB, 2 * RB, 3 * RB, E, O);
+        y2[0] = E.x; y2[1] = E.y; y2[2] = O.x; y2[3] = O.y;
+    }
     if (low_x) {
-        gather4(u2, v1, E, O);
+        make_win(w, sv.tab + (uint32_t)row1 * RB, 0, 0, wu2, lane8);
+        gather4(w, vw1, RB, 2 * RB, 3 * RB, E, O);
         const double h1[4] = {E.x, E.y, O.x, O.y};
 #pragma unroll
         for (int k = 0; k < 4; k++) y1[k] = cont_e(rA, y1[k], h1[k]);
         if (two_v) {
-            gather4(u2, v2, E, O);
+            make_win(w, sv.tab + (uint32_t)row2 * RB, 0, 0, wu2, lane8);
+            gather4(w, vw2, RB, 2 * RB, 3 * RB, E, O);
             const double h2[4] = {E.x, E.y, O.x, O.y};
 #pragma unroll
             for (int k = 0; k < 4; k++) y2[k] = cont_e(rA, y2[k], h2[k]);
@@ -264,16 +276,15 @@ __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, do
     return res;
 }
 
-// output rows of this thread's E / O column pairs (-1 = column not requested)
-struct Rows { int e0, e1, o0, o1; };
-
+// E / O are the column pairs (lane & 1) / the other: put them back in column order and store
 __device__ __forceinline__ void store4(double *__restrict__ out, long long out_stride, long long p,
-                                       const Rows &r, double2 E, double2 O)
+                                       const int row[4], bool odd, double2 E, double2 O)
 {
-    if (r.e0 >= 0) __stcs(out + r.e0 * out_stride + p, E.x);
-    if (r.e1 >= 0) __stcs(out + r.e1 * out_stride + p, E.y);
-    if (r.o0 >= 0) __stcs(out + r.o0 * out_stride + p, O.x);
-    if (r.o1 >= 0) __stcs(out + r.o1 * out_stride + p, O.y);
+    const double c0 = odd ? O.x : E.x, c1 = odd ? O.y : E.y, c2 = odd ? E.x : O.x, c3 = odd ? E.y : O.y;
+    if (row[0] >= 0) __stcs(out + row[0] * out_stride + p, c0);
+    if (row[1] >= 0) __stcs(out + row[1] * out_stride + p, c1);
+    if (row[2] >= 0) __stcs(out + row[2] * out_stride + p, c2);
+    if (row[3] >= 0) __stcs(out + row[3] * out_stride + p, c3);
 }
 
 __global__ void __launch_bounds__(NT_SMEM, 1)
@@ -317,13 +328,9 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     }
     const SmemViews sv = make_views(g, smem);
     const int lane8 = tid & 7;
-    Rows rows;
-    {
-        const int r0 = pl.row[pass][0], r1 = pl.row[pass][1], r2 = pl.row[pass][2], r3 = pl.row[pass][3];
-        const bool odd = lane8 & 1;
-        rows.e0 = odd ? r2 : r0; rows.e1 = odd ? r3 : r1;
-        rows.o0 = odd ? r0 : r2; rows.o1 = odd ? r1 : r3;
-    }
+    const bool odd = lane8 & 1;
+    const uint32_t RB = sv.row_bytes, rb1 = RB, rb2 = 2u * RB, rb3 = 3u * RB;
+    const int row[4] = {pl.row[pass][0], pl.row[pass][1], pl.row[pass][2], pl.row[pass][3]};
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
     int wcount = 0;  // warp-uniform: entries in this warp's list
 
@@ -334,8 +341,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const uint32_t e = s_wlist[warp][lane];
             const long long ps = ((long long)seq + (long long)(e >> 5) * nseq) * NT_SMEM + warp * 32 + (e & 31);
             const Y4 r = slow_point(&g, smem, __ldg(x + ps), __ldg(q2 + ps), lane8);
-            Rows rs = rows;  // the listed point belongs to lane (e & 31): its parity decides nothing here,
-            store4(out, out_stride, ps, rs, r.E, r.O);  // columns follow THIS lane's parity (gather is per lane)
+            store4(out, out_stride, ps, row, odd, r.E, r.O);  // the gather ran on THIS lane: its parity
         }
         __syncwarp();
     };
@@ -354,26 +360,24 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             // ---- locate (LUT guess + exact comparisons where needed), weights, one gather
             const double u = ln_pos(xv), v = ln_pos(qv);
             const int i = locate_x(g, sv, xv, u);
-            int nq, j;
-            const int qo = locate_q(g, sv, qv, v, nq, j);
+            const int gi = locate_q(g, sv, qv, v);
             const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
-            const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)(qo + j) * 128u, lane8);
-            double wu[4];
-            USet us;
-            VSet vs;
-            weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
-            weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vs.w);
-            make_uset(us, i, g.nx, wu, lane8);
-            make_vset(vs, tab, sv.row_bytes, qo, j, nq);
+            const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
+            double wu[4], wv[4], vw[4];
+            const int shx = weights_sh(rx, (u - rx.z0) * rx.inv_dz, wu);
+            const int shq = weights_sh(rq, (v - rq.z0) * rq.inv_dz, wv);
+            rot4(wv, shq & 3, vw);
+            Win w;
+            make_win(w, tab + (uint32_t)(gi - 1 + shq) * RB, i - 1 + shx, shx, wu, lane8);
             double2 E, O;
-            gather4(us, vs, E, O);
-            store4(out, out_stride, p, rows, E, O);
+            gather4(w, vw, rb1, rb2, rb3, E, O);
+            store4(out, out_stride, p, row, odd, E, O);
         }
         const bool invalid = live && !in_range && (!(xv > 0.0) || !(qv > 0.0) || !(xv <= g.x_max) || isinf(qv));
         const bool slow = live && !in_range && !invalid;
         const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
         if (invalid) {
-            store4(out, out_stride, p, rows, make_double2(qnan, qnan), make_double2(qnan, qnan));
+            store4(out, out_stride, p, row, false, make_double2(qnan, qnan), make_double2(qnan, qnan));
             if (pass == 0) atomicAdd(g.n_invalid, 1ULL);
         }
         if (slow_mask) {  // warp-uniform: compact out-of-grid points into this warp's list
@@ -388,7 +392,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 }
 
 static int smem_needed(const GridDev &d) { return d.slice_bytes + d.aux_bytes; }
-static const int STATIC_SMEM = 2304;  // >= the kernel's static shared memory (mbarrier, list)
+static const int STATIC_SMEM = 64 + NT_SMEM * 4 + 256;  // >= the kernel's static shared memory (mbarrier, list)
 
 int pdfb_smem_eligible(const pdfb_grid *g)
 {
