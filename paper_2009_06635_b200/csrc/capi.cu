@@ -1,4 +1,5 @@
 // capi.cu -- the C-ABI of include/pdfb200.h: validation, host grid manager, handles.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdlib>
@@ -97,18 +98,21 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     d.slice_bytes = nq_tot * d.nx4 * 32;
     d.smem_ok = (nx >= 4);
     for (int s = 0; s < n_sub; s++) if (q_offsets[s + 1] - q_offsets[s] < 4) d.smem_ok = 0;
-    if (nq_tot >= 2048 || nx >= 32768) d.smem_ok = 0;  // LUT entry bit budget
-    d.a_xrec = 0;
-    d.a_qrec = d.a_xrec + 128 * nx;
-    d.a_xk = d.a_qrec + 128 * nq_tot;
-    d.a_q2k = d.a_xk + (int)sizeof(double) * nx;
-    d.a_lutx = d.a_q2k + (int)sizeof(double) * nq_tot;
+    if (nq_tot >= 8192 || nx >= 8192) d.smem_ok = 0;  // LUT entry bit budget
+    d.a_lutx = 0;
     d.a_lutq = d.a_lutx + 2 * PDFB_LUT_BINS;
-    d.a_qoff = d.a_lutq + 2 * PDFB_LUT_BINS;
-    d.aux_bytes = (int)align_up(d.a_qoff + sizeof(int) * (n_sub + 1), 16);
+    d.a_xk = d.a_lutq + 2 * PDFB_LUT_BINS;
+    d.a_q2k = d.a_xk + (int)sizeof(double) * nx;
+    d.a_xrec = (int)align_up(d.a_q2k + sizeof(double) * nq_tot, 128);
+    d.pre_bytes = d.a_xrec + 128 * nx;            // the slice starts here, 128-byte aligned
+    d.a_qrec = 0;
+    // a stencil may reach one row plus three knots past the table: keep that much finite data there
+    d.post_bytes = (int)align_up((size_t)std::max(128 * nq_tot, d.nx4 * 32 + 128), 128);
+    if (128 * nx < d.nx4 * 32 + 32) d.smem_ok = 0;  // (never: 128 nx >= 32 nx4 + 32 for nx >= 2)
+    const int aux_bytes = d.pre_bytes + d.post_bytes;
     size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid, 128);
     size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups, 128);
-    size_t total = o_aux + d.aux_bytes;
+    size_t total = o_aux + aux_bytes;
     char *blob = nullptr;
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
     g->blob = blob; g->blob_bytes = total;
@@ -132,7 +136,7 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         // K1: interval records for the x knots and for each sub-grid's Q^2 knots
         int xoff[2] = {0, nx};
         {   // host part of the aux block: raw knots, search LUTs, sub-grid of each Q^2 knot
-            std::vector<unsigned char> aux(d.aux_bytes, 0);
+            std::vector<unsigned char> aux(aux_bytes, 0);
             memcpy(aux.data() + d.a_xk, x_knots, sizeof(double) * nx);
             memcpy(aux.data() + d.a_q2k, h_q2.data(), sizeof(double) * nq_tot);
             unsigned short *lx = (unsigned short *)(aux.data() + d.a_lutx);
@@ -140,36 +144,34 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
             const double *U = h_z.data(), *V = h_z.data() + nx;
             d.lutx_u0 = U[0]; d.lutx_inv_h = PDFB_LUT_BINS / (U[nx - 1] - U[0]);
             d.lutq_v0 = V[0]; d.lutq_inv_h = PDFB_LUT_BINS / (V[nq_tot - 1] - V[0]);
-            const double hx = (U[nx - 1] - U[0]) / PDFB_LUT_BINS, hq = (V[nq_tot - 1] - V[0]) / PDFB_LUT_BINS;
-            const double mx = 1e-6 * hx, mq = 1e-6 * hq;  // safety margin around bin edges
-            for (int b = 0; b < PDFB_LUT_BINS; b++) {
-                double lo = U[0] + b * hx - mx, hi = U[0] + (b + 1) * hx + mx;
-                int i = 0, straddle = 0;
-                for (int k = 1; k <= nx - 2; k++) {
-                    if (U[k] <= lo) i = k;
-                    else if (U[k] <= hi) straddle = 1;
+            // LUT over [Z_0, Z_{nk-1}] for knots 0..kmax, raw values R: encoding in pdfb_internal.cuh
+            auto fill = [](unsigned short *lut, const double *Z, const double *R, int nk, int kmax) {
+                const double h = (Z[nk - 1] - Z[0]) / PDFB_LUT_BINS, mg = 1e-6 * h;  // safety margin at bin edges
+                for (int b = 0; b < PDFB_LUT_BINS; b++) {
+                    const double lo = Z[0] + b * h - mg, hi = Z[0] + (b + 1) * h + mg;
+                    int m0 = 0, first = -1, last = -1, multi = 0;
+                    for (int k = 1; k <= kmax; k++) {
+                        if (Z[k] <= lo) m0 = k;
+                        else if (Z[k] <= hi) {
+                            if (first < 0) first = k;
+                            else if (R[k] != R[first]) multi = 1;
+                            last = k;
+                        }
+                    }
+                    int delta = (first >= 0 && !multi) ? last - m0 : 0;
+                    if (delta > 3) { multi = 1; delta = 0; }
+                    lut[b] = (unsigned short)((m0 << 3) | (delta << 1) | multi);
                 }
-                lx[b] = (unsigned short)((i << 1) | straddle);
-            }
-            for (int b = 0; b < PDFB_LUT_BINS; b++) {
-                double lo = V[0] + b * hq - mq, hi = V[0] + (b + 1) * hq + mq;
-                int m = 0, straddle = 0;
-                for (int k = 1; k <= nq_tot - 1; k++) {
-                    if (V[k] <= lo) m = k;
-                    else if (V[k] <= hi) straddle = 1;
-                }
-                int sub = 0;
-                for (int s2 = 0; s2 < n_sub; s2++) if (q_offsets[s2] <= m) sub = s2;
-                lq[b] = (unsigned short)((m << 5) | (sub << 1) | straddle);
-            }
-            memcpy(aux.data() + d.a_qoff, q_offsets, sizeof(int) * (n_sub + 1));
-            if (cudaMemcpy(blob + o_aux, aux.data(), d.aux_bytes, cudaMemcpyHostToDevice) != cudaSuccess) { rc = PDFB_ECUDA; break; }
+            };
+            fill(lx, U, x_knots, nx, nx - 2);          // the last x knot starts no interval
+            fill(lq, V, h_q2.data(), nq_tot, nq_tot - 1);  // concatenated Q^2 knots; clamped after the search
+            if (cudaMemcpy(blob + o_aux, aux.data(), aux_bytes, cudaMemcpyHostToDevice) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         }
         rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec),
                                 (IntervalRec32 *)(blob + o_aux + d.a_xrec), 1, xoff, 0);
         if (rc) break;
         rc = pdfb_setup_records((const double *)(blob + o_z) + nx, (IntervalRec *)(blob + o_qrec),
-                                (IntervalRec32 *)(blob + o_aux + d.a_qrec), n_sub, d.q_off, 0);
+                                (IntervalRec32 *)(blob + o_aux + d.pre_bytes + d.a_qrec), n_sub, d.q_off, 0);
         if (rc) break;
         // K1: value table re-layout, sub-grid by sub-grid
         long long src = 0;
@@ -198,12 +200,6 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         if (cudaMemcpy(&rC, blob + o_qrec + sizeof(IntervalRec) * jC, sizeof(rC), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         d.jC = jC;
         weights4(rC, (h_z[nx + nq_tot] - rC.z0) * rC.inv_dz, d.wvC);
-        // window form for the shared-memory path: 4 consecutive rows inside sub-grid 0; in an edge
-        // interval the window is shifted by one and the weights rotate (the wrapped weight is 0)
-        int shC = (jC == 0 ? 1 : 0) - (jC == nq0 - 2 ? 1 : 0);
-        if (nq0 < 4) shC = 0;  // such grids never take the shared-memory path
-        d.rowC = jC - 1 + shC;
-        for (int b = 0; b < 4; b++) d.wvCw[b] = d.wvC[(b + shC + 4) & 3];
     } while (0);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
     if (rc) { cudaFree(blob); delete g; return rc; }

@@ -101,8 +101,6 @@ struct GridDev {
     double Va, Vb, inv_dVab;           // ln of the last two Q^2 knots, 1/(Vb-Va)
     int jC;                            // interval of 1.01*q2_min in sub-grid 0
     double wvC[4];                     // its four v weights (fixed per grid), stencil order j-1..j+2
-    int rowC;                          // first row of its 4-row window inside sub-grid 0 (smem path)
-    double wvCw[4];                    // the same weights in window order
     const double *xk;                  // [nx] x knots
     const double *q2k;                 // [nq_tot] Q^2 knots
     const IntervalRec *xrec;           // [nx-1]
@@ -114,17 +112,24 @@ struct GridDev {
     int n_groups, nx4;                 // groups of 4 value columns; nx padded to a multiple of 4
     int slice_bytes;                   // one group's slice: nq_tot * nx4 * 32 B
     const double *valg;                // [group][s][iq][ix4][4]
-    const unsigned char *aux;          // aux block, copied verbatim into shared memory
-    int aux_bytes;
-    int a_xk, a_q2k, a_xrec, a_qrec, a_lutx, a_lutq, a_qoff;  // byte offsets inside aux
+    const unsigned char *aux;          // [pre | post] blocks, copied verbatim around the slice
+    int pre_bytes, post_bytes;         // shared memory = [pre | slice | post]
+    int a_xk, a_q2k, a_lutx, a_lutq, a_xrec;  // byte offsets inside pre (a_xrec is its tail)
+    int a_qrec;                        // byte offset inside post (its head)
     double lutx_u0, lutx_inv_h, lutq_v0, lutq_inv_h;
 };
 #define PDFB_LUT_BINS 512
-// aux block: xrec/qrec = 128-byte lines holding 4 copies of the 32-byte IntervalRec32 of an
-// interval; lutx[b] = (i << 1) | straddle, lutq[b] = (m << 5) | (s << 1) | straddle, where i / m
-// is the last knot at or left of the bin's left edge (m indexes the concatenated Q^2 knots,
-// s its sub-grid) and `straddle` says a knot lies inside the bin, so the guess must be
-// corrected by comparisons on the raw knots; qoff = the sub-grid knot offsets (ints).
+// Shared-memory image of the smem path: [pre | slice | post].
+//   pre  = lutx, lutq, raw x knots, raw Q^2 knots, then xrec;   post = qrec, then zero padding.
+// xrec/qrec = 128-byte lines holding 4 copies of the 32-byte IntervalRec32 of an interval (qrec is
+// indexed by the concatenated Q^2 knot index).  The slice is bracketed by xrec and qrec ON PURPOSE:
+// the 4x4 stencil of an edge interval reaches one row / one knot outside the table with weight
+// exactly 0 (one-sided rule, reading O2), and what it reads there must be finite doubles.
+// lut[b] = (m0 << 3) | (delta << 1) | multi, where m0 is the last knot at or left of the bin's
+// left edge; if exactly one knot value lies inside the bin, delta = (index of its last copy) - m0
+// and the interval is m0 + delta iff knots[m0 + delta] <= the raw coordinate, else m0; `multi`
+// (several distinct knots in the bin) asks for the comparison loop.  A Q^2 threshold is stored
+// twice in the concatenated list, so a point on it lands on the upper copy (reading Q2).
 
 // 32-byte interval record of the shared-memory path: the remaining coefficients follow from
 // "a derivative annihilates constants": aL1 = (aLm == 0 ? 1 : 1/2), aL0 = -(aLm + aL1),

@@ -9,12 +9,13 @@
 //     staged once per CTA by TMA bulk copies.  Each persistent CTA serves one group for all
 //     points of its tiles, so it writes whole flavour rows with coalesced stores and no point
 //     ever has to be re-ordered;
-//   * the 4x4 stencil is always read as a WINDOW of 4 consecutive rows x 4 consecutive knots that
-//     lies inside the knot array / the sub-grid: in an edge interval the window is shifted by one
-//     and the weights are rotated cyclically, which is exact because the knot that wraps around
-//     carries weight exactly 0 (one-sided derivative rule, reading O2).  Rows of a window are a
-//     uniform stride apart, so the 32 loads of a point use 8 per-lane addresses + 3 uniform
-//     offsets (LDS [R+UR]) and no address arithmetic;
+//   * the 4x4 stencil is always read as 4 consecutive rows x 4 consecutive knots, rows i-1..i+2 of
+//     the concatenated table.  In an edge interval the stencil reaches one row / one knot outside
+//     the knot array or the sub-grid; that knot carries weight exactly 0 (one-sided derivative
+//     rule, reading O2), so whatever finite number sits there contributes nothing: a neighbouring
+//     sub-grid's row, the next row's first knot, or the interval records that bracket the slice in
+//     shared memory.  Rows are a uniform stride apart, so the 32 loads of a point use 8 per-lane
+//     addresses + 3 uniform offsets (LDS [R+UR]) and no address arithmetic;
 //   * one window row (4 knots x 4 flavours) is 128 contiguous bytes = 8 chunks of 16 B that
 //     cover all 8 bank groups.  Lane l reads them in the rotated order c = (s + l - 2*node0) & 7,
 //     so at every step the 8 lanes of a quarter-warp hit 8 distinct bank groups whatever cells
@@ -52,12 +53,12 @@ __device__ __forceinline__ double cont_e(double r, double yL, double yH)  // rea
     return fma(r, yH - yL, yL);
 }
 
-// The four 1-D weights of knots m-1..m+2 (stencil order) from the 32-byte interval record, and
-// the window shift sh: the window starts at knot m-1+sh, sh = +1 in the first interval of the
-// array (aLm == 0: knot m-1 does not exist), -1 in the last (aHp == 0), else 0.
-__device__ __forceinline__ int weights_sh(const IntervalRec32 &r, double t, double w[4])
+// The four 1-D weights of knots m-1..m+2 from the 32-byte interval record.  aLm == 0 marks the
+// first interval of the knot array (knot m-1 does not exist, weight exactly 0), aHp == 0 the last.
+__device__ __forceinline__ void weights_rec32(const IntervalRec32 &r, double t, double w[4])
 {
-    const bool first = (r.aLm == 0.0), last = (r.aHp == 0.0);
+    // exact zero tests on the high words (the records hold +0.0 there), off the FP64 pipe
+    const bool first = (__double2hiint(r.aLm) << 1) == 0, last = (__double2hiint(r.aHp) << 1) == 0;
     double t2 = t * t, t3 = t2 * t;
     double h01 = 3.0 * t2 - 2.0 * t3;
     double h00 = 1.0 - h01;
@@ -69,7 +70,6 @@ __device__ __forceinline__ int weights_sh(const IntervalRec32 &r, double t, doub
     w[1] = fma(h11, aH0, fma(h10, aL0, h00));
     w[2] = fma(h11, aH1, fma(h10, aL1, h01));
     w[3] = h11 * r.aHp;
-    return (first ? 1 : 0) - (last ? 1 : 0);
 }
 
 // o[k] = w[(k + r) & 3]
@@ -82,25 +82,25 @@ __device__ __forceinline__ void rot4(const double w[4], int r, double o[4])
     for (int k = 0; k < 4; k++) o[k] = (r & 2) ? a[(k + 2) & 3] : a[k];
 }
 
-// One (x window, row window) pair of a point.  The 128-byte run of window knots node0..node0+3
-// (4 columns each) holds chunk c = 2*(knot - node0) + (column pair).  Lane l reads, at step s,
+// The x side of a point's stencil.  The 128-byte run of knots node0..node0+3 (node0 = i-1, 4
+// columns each) holds chunk c = 2*(knot - node0) + (column pair).  Lane l reads, at step s,
 //   c(s) = ((s + rot) & 7) ^ (l & 1),   rot = ((l & 6) - 2*node0) & 7   (even),
 // which puts the 8 lanes of a quarter-warp on 8 distinct bank groups at every step.  Steps 2k and
-// 2k+1 both belong to window knot (k + rot/2) & 3, so one rotated weight W[k] serves both; even
-// steps deliver column pair (l & 1), odd steps the other pair (swapped back before the store).
+// 2k+1 both belong to knot (k + rot/2) & 3, so one rotated weight W[k] serves both; even steps
+// deliver column pair (l & 1), odd steps the other pair (swapped back before the store).
 struct Win { uint32_t a[8]; double W[4]; };
 
-// row0 = shared address of window row 0; wu = x weights in stencil order, shx their window shift
-__device__ __forceinline__ void make_win(Win &u, uint32_t row0, int node0, int shx, const double wu[4], int lane8)
+// row0 = shared address of stencil row 0 (table row gi-1); wu = x weights of knots node0..node0+3
+__device__ __forceinline__ void make_win(Win &u, uint32_t row0, int node0, const double wu[4], int lane8)
 {
     const int rot2 = ((lane8 >> 1) - node0) & 3;
-    const uint32_t base = row0 + (uint32_t)node0 * 32u + ((uint32_t)(lane8 & 1) << 4);
+    const uint32_t base = row0 + (uint32_t)(node0 * 32) + ((uint32_t)(lane8 & 1) << 4);
 #pragma unroll
     for (int k = 0; k < 4; k++) {
         u.a[2 * k] = base + ((uint32_t)((k + rot2) & 3) << 5);
         u.a[2 * k + 1] = u.a[2 * k] ^ 16u;
     }
-    rot4(wu, (rot2 + shx) & 3, u.W);
+    rot4(wu, rot2, u.W);
 }
 
 // sum_b vw[b] * sum_k W[k] * V[window row b][window knot][cols] -> E = column pair (lane & 1), O = the other
@@ -133,18 +133,19 @@ struct SmemViews {
     const unsigned short *lutx, *lutq;
 };
 
+// shared memory = [pre | slice | post] (pdfb_internal.cuh)
 __device__ __forceinline__ SmemViews make_views(const GridDev &g, unsigned char *smem)
 {
     SmemViews sv;
-    unsigned char *s_aux = smem + g.slice_bytes;
-    sv.tab = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(smem);
+    sv.tab = s0 + (uint32_t)g.pre_bytes;
     sv.row_bytes = (uint32_t)g.nx4 * 32u;
-    sv.xrec = sv.tab + (uint32_t)(g.slice_bytes + g.a_xrec);
+    sv.xrec = s0 + (uint32_t)g.a_xrec;
     sv.qrec = sv.tab + (uint32_t)(g.slice_bytes + g.a_qrec);
-    sv.xk = reinterpret_cast<const double *>(s_aux + g.a_xk);
-    sv.q2k = reinterpret_cast<const double *>(s_aux + g.a_q2k);
-    sv.lutx = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutx);
-    sv.lutq = reinterpret_cast<const unsigned short *>(s_aux + g.a_lutq);
+    sv.xk = reinterpret_cast<const double *>(smem + g.a_xk);
+    sv.q2k = reinterpret_cast<const double *>(smem + g.a_q2k);
+    sv.lutx = reinterpret_cast<const unsigned short *>(smem + g.a_lutx);
+    sv.lutq = reinterpret_cast<const unsigned short *>(smem + g.a_lutq);
     return sv;
 }
 
@@ -162,32 +163,38 @@ __device__ __forceinline__ IntervalRec32 load_rec4(uint32_t line, int lane8)
     return r;
 }
 
-// interval of x: LUT guess, corrected by comparisons on the raw knots where a knot lies in the bin
-__device__ __forceinline__ int locate_x(const GridDev &g, const SmemViews &sv, double xv, double u)
+// Interval search: LUT guess (pdfb_internal.cuh) + at most one comparison on the raw knots; bins
+// holding several distinct knots take the comparison loop.  Returns the last m <= kmax with
+// knots[m] <= val (the result is defined by the comparisons, reading Q5).
+__device__ __forceinline__ int locate(const unsigned short *lut, const double *knots, int kmax, double val,
+                                      double z, double z0, double inv_h)
 {
-    int b = min(max((int)((u - g.lutx_u0) * g.lutx_inv_h), 0), PDFB_LUT_BINS - 1);
-    int e = sv.lutx[b], i = e >> 1;
+    const int b = min(max((int)((z - z0) * inv_h), 0), PDFB_LUT_BINS - 1);
+    const int e = lut[b], d = (e >> 1) & 3;
+    int m = e >> 3;
+    if (d) { if (knots[m + d] <= val) m += d; }
     if (e & 1)
-        while (i < g.nx - 2 && sv.xk[i + 1] <= xv) ++i;
-    return i;
+        while (m < kmax && knots[m + 1] <= val) ++m;
+    return m;
 }
 
-// Interval of Q^2 as an index into the CONCATENATED knot list: m = the last knot <= Q^2.  A
-// threshold is stored twice (last knot of the lower sub-grid, first of the upper), so a point on
-// it lands on the upper copy (reading Q2) and the lower copy is never an interval start; only
-// Q^2 = q2_max needs the clamp.  Interval records and table rows use the same index.
+__device__ __forceinline__ int locate_x(const GridDev &g, const SmemViews &sv, double xv, double u)
+{
+    return locate(sv.lutx, sv.xk, g.nx - 2, xv, u, g.lutx_u0, g.lutx_inv_h);
+}
+
+// Interval of Q^2 as an index into the CONCATENATED knot list.  A threshold is stored twice (last
+// knot of the lower sub-grid, first of the upper), so a point on it lands on the upper copy
+// (reading Q2) and the lower copy never starts an interval; only Q^2 = q2_max needs the clamp.
+// Interval records and table rows use the same index.
 __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, double qv, double v)
 {
-    int b = min(max((int)((v - g.lutq_v0) * g.lutq_inv_h), 0), PDFB_LUT_BINS - 1);
-    int e = sv.lutq[b], m = e >> 5;
-    if (e & 1)
-        while (m < g.nq_tot - 1 && sv.q2k[m + 1] <= qv) ++m;
-    return min(m, g.nq_tot - 2);
+    return min(locate(sv.lutq, sv.q2k, g.nq_tot - 1, qv, v, g.lutq_v0, g.lutq_inv_h), g.nq_tot - 2);
 }
 
 struct Y4 { double2 E, O; };  // column pair (lane & 1) and the other pair
 
-// points outside the grid (readings O4/O5): up to 2 x-sets times 2 row windows
+// points outside the grid (readings O4/O5): up to 2 x-sets times 2 row sets
 __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
 {
     const GridDev &g = *gp;
@@ -195,62 +202,60 @@ __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, do
     const uint32_t RB = sv.row_bytes;
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
     // ---- x: one weight set in range, else the two one-hot sets of knots 0 and 1 (rule A)
-    double wu1[4] = {1.0, 0.0, 0.0, 0.0}, wu2[4] = {0.0, 1.0, 0.0, 0.0};  // window knots 0..3, shift 0
-    int node0 = 0, shx = 0;
+    double wu1[4] = {1.0, 0.0, 0.0, 0.0}, wu2[4] = {0.0, 1.0, 0.0, 0.0};  // knots 0..3
+    int node0 = 0;
     double rA = 0.0;
     if (!low_x) {
         const double u = ln_pos(xv);
         const int i = locate_x(g, sv, xv, u);
         const IntervalRec32 r = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
-        shx = weights_sh(r, (u - r.z0) * r.inv_dz, wu1);
-        node0 = i - 1 + shx;
+        weights_rec32(r, (u - r.z0) * r.inv_dz, wu1);
+        node0 = i - 1;
     } else {
         rA = (pdfb_ln(xv) - g.U0) * g.inv_dU01;
     }
-    // ---- rows: one window in range, else two probes (rules B, C)
+    // ---- rows: one stencil in range, else two probes (rules B, C); row = table row of stencil row 0
     int row1, row2;
     double vw1[4], vw2[4];
     double rB = 0.0;
-    if (high_q) {  // the last two Q^2 knots of the last sub-grid: rows 2 and 3 of its last window
+    if (high_q) {  // the last two Q^2 knots of the last sub-grid
         rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
         row1 = row2 = g.nq_tot - 4;
         vw1[0] = vw1[1] = vw1[3] = 0.0; vw1[2] = 1.0;
         vw2[0] = vw2[1] = vw2[2] = 0.0; vw2[3] = 1.0;
-    } else if (low_q) {  // q_min (row 0 of sub-grid 0) and 1.01 q_min (fixed window and weights)
+    } else if (low_q) {  // q_min (row 0 of sub-grid 0) and 1.01 q_min (fixed interval and weights)
         row1 = 0;
         vw1[0] = 1.0; vw1[1] = vw1[2] = vw1[3] = 0.0;
-        row2 = g.rowC;
+        row2 = g.jC - 1;
 #pragma unroll
-        for (int b = 0; b < 4; b++) vw2[b] = g.wvCw[b];
+        for (int b = 0; b < 4; b++) vw2[b] = g.wvC[b];
     } else {
         const double v = ln_pos(qv);
         const int gi = locate_q(g, sv, qv, v);
         const IntervalRec32 r = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
-        double wv[4];
-        const int shq = weights_sh(r, (v - r.z0) * r.inv_dz, wv);
-        rot4(wv, shq & 3, vw1);
-        row1 = row2 = gi - 1 + shq;
+        weights_rec32(r, (v - r.z0) * r.inv_dz, vw1);
+        row1 = row2 = gi - 1;
     }
     const bool two_v = high_q || low_q;
     double y1[4], y2[4] = {0.0, 0.0, 0.0, 0.0};
     double2 E, O;
     Win w;
-    make_win(w, sv.tab + (uint32_t)row1 * RB, node0, shx, wu1, lane8);
+    make_win(w, sv.tab + (uint32_t)(row1 * (int)RB), node0, wu1, lane8);
     gather4(w, vw1, RB, 2 * RB, 3 * RB, E, O);
     y1[0] = E.x; y1[1] = E.y; y1[2] = O.x; y1[3] = O.y;
     if (two_v) {
-        make_win(w, sv.tab + (uint32_t)row2 * RB, node0, shx, wu1, lane8);
+        make_win(w, sv.tab + (uint32_t)(row2 * (int)RB), node0, wu1, lane8);
         gather4(w, vw2, RB, 2 * RB, 3 * RB, E, O);
         y2[0] = E.x; y2[1] = E.y; y2[2] = O.x; y2[3] = O.y;
     }
     if (low_x) {
-        make_win(w, sv.tab + (uint32_t)row1 * RB, 0, 0, wu2, lane8);
+        make_win(w, sv.tab + (uint32_t)(row1 * (int)RB), 0, wu2, lane8);
         gather4(w, vw1, RB, 2 * RB, 3 * RB, E, O);
         const double h1[4] = {E.x, E.y, O.x, O.y};
 #pragma unroll
         for (int k = 0; k < 4; k++) y1[k] = cont_e(rA, y1[k], h1[k]);
         if (two_v) {
-            make_win(w, sv.tab + (uint32_t)row2 * RB, 0, 0, wu2, lane8);
+            make_win(w, sv.tab + (uint32_t)(row2 * (int)RB), 0, wu2, lane8);
             gather4(w, vw2, RB, 2 * RB, 3 * RB, E, O);
             const double h2[4] = {E.x, E.y, O.x, O.y};
 #pragma unroll
@@ -298,8 +303,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int pass = blockIdx.x % pl.n, seq = blockIdx.x / pl.n, nseq = gridDim.x / pl.n;
     if (seq >= nseq) return;
-    unsigned char *s_aux = smem + g.slice_bytes;
-    const uint32_t tab = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t tab = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)g.pre_bytes;
     const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&mbar);
 
     // ---- stage this CTA's flavour-group slice with TMA bulk copies; small tables by plain loads
@@ -317,8 +321,13 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                          ::"r"(tab + o), "l"(src + o), "r"(bytes), "r"(mb) : "memory");
         }
     }
-    for (int e = tid; e < g.aux_bytes / 16; e += NT_SMEM)
-        reinterpret_cast<int4 *>(s_aux)[e] = __ldg(reinterpret_cast<const int4 *>(g.aux) + e);
+    {   // pre and post blocks around the slice (both multiples of 128 bytes)
+        const int4 *src = reinterpret_cast<const int4 *>(g.aux);
+        int4 *pre = reinterpret_cast<int4 *>(smem), *post = reinterpret_cast<int4 *>(smem + g.pre_bytes + g.slice_bytes);
+        const int npre = g.pre_bytes / 16, npost = g.post_bytes / 16;
+        for (int e = tid; e < npre; e += NT_SMEM) pre[e] = __ldg(src + e);
+        for (int e = tid; e < npost; e += NT_SMEM) post[e] = __ldg(src + npre + e);
+    }
     __syncthreads();
     {
         uint32_t done = 0;
@@ -363,12 +372,11 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const int gi = locate_q(g, sv, qv, v);
             const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
             const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
-            double wu[4], wv[4], vw[4];
-            const int shx = weights_sh(rx, (u - rx.z0) * rx.inv_dz, wu);
-            const int shq = weights_sh(rq, (v - rq.z0) * rq.inv_dz, wv);
-            rot4(wv, shq & 3, vw);
+            double wu[4], vw[4];
+            weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
+            weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vw);
             Win w;
-            make_win(w, tab + (uint32_t)(gi - 1 + shq) * RB, i - 1 + shx, shx, wu, lane8);
+            make_win(w, tab + (uint32_t)((gi - 1) * (int)RB), i - 1, wu, lane8);
             double2 E, O;
             gather4(w, vw, rb1, rb2, rb3, E, O);
             store4(out, out_stride, p, row, odd, E, O);
@@ -391,7 +399,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     if (wcount) flush(wcount);
 }
 
-static int smem_needed(const GridDev &d) { return d.slice_bytes + d.aux_bytes; }
+static int smem_needed(const GridDev &d) { return d.pre_bytes + d.slice_bytes + d.post_bytes; }
 static const int STATIC_SMEM = 64 + NT_SMEM * 4 + 256;  // >= the kernel's static shared memory (mbarrier, list)
 
 int pdfb_smem_eligible(const pdfb_grid *g)
