@@ -69,7 +69,9 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
         if (qv >= A.q2_min && qv <= A.q2_max) {
             const double v = pdfb_ln(qv);
             int b = min(max((int)((v - A.lut_v0) * A.lut_inv_h), 0), PDFB_LUT_BINS - 1);
-            int e = lut[b], m = e >> 1;
+            const int e = lut[b], d = (e >> 1) & 3;
+            int m = e >> 3;
+            if (d) { if (q2k[m + d] <= qv) m += d; }
             if (e & 1)
                 while (m < A.K - 1 && q2k[m + 1] <= qv) ++m;
             m = min(m, A.K - 2);  // Q^2 = last node: last interval, t = 1

@@ -28,6 +28,28 @@ extern "C" const char *pdfb_strerror(int code)
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Search LUT over [Z_0, Z_{nk-1}] (ln knots) for knots 0..kmax with raw values R; the entry
+// encoding is described in pdfb_internal.cuh.
+void pdfb_fill_lut(unsigned short *lut, const double *Z, const double *R, int nk, int kmax)
+{
+    const double h = (Z[nk - 1] - Z[0]) / PDFB_LUT_BINS, mg = 1e-6 * h;  // safety margin at bin edges
+    for (int b = 0; b < PDFB_LUT_BINS; b++) {
+        const double lo = Z[0] + b * h - mg, hi = Z[0] + (b + 1) * h + mg;
+        int m0 = 0, first = -1, last = -1, multi = 0;
+        for (int k = 1; k <= kmax; k++) {
+            if (Z[k] <= lo) m0 = k;
+            else if (Z[k] <= hi) {
+                if (first < 0) first = k;
+                else if (R[k] != R[first]) multi = 1;
+                last = k;
+            }
+        }
+        int delta = (first >= 0 && !multi) ? last - m0 : 0;
+        if (delta > 3) { multi = 1; delta = 0; }
+        lut[b] = (unsigned short)((m0 << 3) | (delta << 1) | multi);
+    }
+}
+
 // ------------------------------------------------------------------------------ PDF grid
 extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
                              const double *q_knots, int n_pid, const int *pids, const double *values,
@@ -144,27 +166,8 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
             const double *U = h_z.data(), *V = h_z.data() + nx;
             d.lutx_u0 = U[0]; d.lutx_inv_h = PDFB_LUT_BINS / (U[nx - 1] - U[0]);
             d.lutq_v0 = V[0]; d.lutq_inv_h = PDFB_LUT_BINS / (V[nq_tot - 1] - V[0]);
-            // LUT over [Z_0, Z_{nk-1}] for knots 0..kmax, raw values R: encoding in pdfb_internal.cuh
-            auto fill = [](unsigned short *lut, const double *Z, const double *R, int nk, int kmax) {
-                const double h = (Z[nk - 1] - Z[0]) / PDFB_LUT_BINS, mg = 1e-6 * h;  // safety margin at bin edges
-                for (int b = 0; b < PDFB_LUT_BINS; b++) {
-                    const double lo = Z[0] + b * h - mg, hi = Z[0] + (b + 1) * h + mg;
-                    int m0 = 0, first = -1, last = -1, multi = 0;
-                    for (int k = 1; k <= kmax; k++) {
-                        if (Z[k] <= lo) m0 = k;
-                        else if (Z[k] <= hi) {
-                            if (first < 0) first = k;
-                            else if (R[k] != R[first]) multi = 1;
-                            last = k;
-                        }
-                    }
-                    int delta = (first >= 0 && !multi) ? last - m0 : 0;
-                    if (delta > 3) { multi = 1; delta = 0; }
-                    lut[b] = (unsigned short)((m0 << 3) | (delta << 1) | multi);
-                }
-            };
-            fill(lx, U, x_knots, nx, nx - 2);          // the last x knot starts no interval
-            fill(lq, V, h_q2.data(), nq_tot, nq_tot - 1);  // concatenated Q^2 knots; clamped after the search
+            pdfb_fill_lut(lx, U, x_knots, nx, nx - 2);          // the last x knot starts no interval
+            pdfb_fill_lut(lq, V, h_q2.data(), nq_tot, nq_tot - 1);  // concatenated Q^2 knots; clamped after the search
             if (cudaMemcpy(blob + o_aux, aux.data(), aux_bytes, cudaMemcpyHostToDevice) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         }
         rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec),

@@ -67,19 +67,10 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
     if (!rc) rc = pdfb_setup_alphas_fast((const IntervalRec *)(blob + o_rec), (const double *)(blob + o_a),
                                          (unsigned char *)(blob + o_fast), n_sub, d.off, 0);
     if (!rc && cudaMemcpy(h_z.data(), blob + o_z, sizeof(double) * n_knots, cudaMemcpyDeviceToHost) != cudaSuccess) rc = PDFB_ECUDA;
-    if (!rc) {  // LUT over ln Q^2: (m << 1) | straddle, m = last node at or left of the bin's left edge
+    if (!rc) {  // LUT over ln Q^2 (encoding in pdfb_internal.cuh); a repeated node lands on its upper copy
         std::vector<unsigned short> lut(PDFB_LUT_BINS);
-        const double h = (h_z[n_knots - 1] - h_z[0]) / PDFB_LUT_BINS, mg = 1e-6 * h;
         d.lut_v0 = h_z[0]; d.lut_inv_h = PDFB_LUT_BINS / (h_z[n_knots - 1] - h_z[0]);
-        for (int b = 0; b < PDFB_LUT_BINS; b++) {
-            double lo = h_z[0] + b * h - mg, hi = h_z[0] + (b + 1) * h + mg;
-            int m = 0, straddle = 0;
-            for (int k = 1; k <= n_knots - 1; k++) {
-                if (h_z[k] <= lo) m = k;
-                else if (h_z[k] <= hi) straddle = 1;
-            }
-            lut[b] = (unsigned short)((m << 1) | straddle);
-        }
+        pdfb_fill_lut(lut.data(), h_z.data(), h_q2.data(), n_knots, n_knots - 1);
         if (cudaMemcpy(blob + o_fast + d.f_q2k, h_q2.data(), sizeof(double) * n_knots, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(blob + o_fast + d.f_lut, lut.data(), 2 * PDFB_LUT_BINS, cudaMemcpyHostToDevice) != cudaSuccess)
             rc = PDFB_ECUDA;

@@ -176,6 +176,9 @@ struct pdfb_alphas {
     cudaStream_t streams[2];
 };
 
+// search LUT (capi.cu); encoding above
+void pdfb_fill_lut(unsigned short *lut, const double *Z, const double *R, int nk, int kmax);
+
 // launch accounting (capi.cu)
 void pdfb_count_launch(int n);
 

@@ -34,7 +34,10 @@ struct PassList {
 };
 
 #ifndef NT_SMEM
-#define NT_SMEM 512
+#define NT_SMEM 512   // threads per CTA (one CTA per SM: the slice fills shared memory)
+#endif
+#ifndef PPT_SMEM
+#define PPT_SMEM 1    // points per thread and tile
 #endif
 
 __device__ __forceinline__ double2 lds128(uint32_t addr)
@@ -344,11 +347,14 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     int wcount = 0;  // warp-uniform: entries in this warp's list
 
     // evaluate the listed out-of-grid points of this warp with (mostly) full lanes
+    constexpr int TILE = NT_SMEM * PPT_SMEM;
     auto flush = [&](int count) {
         __syncwarp();
         if (lane < count) {
-            const uint32_t e = s_wlist[warp][lane];
-            const long long ps = ((long long)seq + (long long)(e >> 5) * nseq) * NT_SMEM + warp * 32 + (e & 31);
+            const uint32_t e = s_wlist[warp][lane];  // (iteration * PPT + k) << 5 | lane
+            const uint32_t ik = e >> 5;
+            const long long ps = ((long long)seq + (long long)(ik / PPT_SMEM) * nseq) * TILE + (ik % PPT_SMEM) * NT_SMEM +
+                                 warp * 32 + (e & 31);
             const Y4 r = slow_point(&g, smem, __ldg(x + ps), __ldg(q2 + ps), lane8);
             store4(out, out_stride, ps, row, odd, r.E, r.O);  // the gather ran on THIS lane: its parity
         }
@@ -357,44 +363,68 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 
     // software pipeline: the next tile's coordinates are in flight while this tile is evaluated
     long long tile = seq;
-    long long p = tile * NT_SMEM + tid;
-    double xv = (p < n) ? __ldg(x + p) : 1.0, qv = (p < n) ? __ldg(q2 + p) : 1.0;
-    for (uint32_t it = 0; tile * NT_SMEM < n; tile += nseq, ++it) {
-        p = tile * NT_SMEM + tid;
-        const long long pn = p + (long long)nseq * NT_SMEM;
-        const double xn = (pn < n) ? __ldg(x + pn) : 1.0, qn = (pn < n) ? __ldg(q2 + pn) : 1.0;
-        const bool live = p < n;
-        const bool in_range = live && xv >= g.x_min && xv <= g.x_max && qv >= g.q2_min && qv <= g.q2_max;
-        if (in_range) {
-            // ---- locate (LUT guess + exact comparisons where needed), weights, one gather
-            const double u = ln_pos(xv), v = ln_pos(qv);
-            const int i = locate_x(g, sv, xv, u);
-            const int gi = locate_q(g, sv, qv, v);
-            const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
-            const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
-            double wu[4], vw[4];
-            weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
-            weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vw);
-            Win w;
-            make_win(w, tab + (uint32_t)((gi - 1) * (int)RB), i - 1, wu, lane8);
-            double2 E, O;
-            gather4(w, vw, rb1, rb2, rb3, E, O);
-            store4(out, out_stride, p, row, odd, E, O);
+    double xv[PPT_SMEM], qv[PPT_SMEM];
+#pragma unroll
+    for (int k = 0; k < PPT_SMEM; k++) {
+        const long long p = tile * TILE + k * NT_SMEM + tid;
+        xv[k] = (p < n) ? __ldg(x + p) : 1.0; qv[k] = (p < n) ? __ldg(q2 + p) : 1.0;
+    }
+    for (uint32_t it = 0; tile * TILE < n; tile += nseq, ++it) {
+        const long long p0 = tile * TILE + tid;
+        double xn[PPT_SMEM], qn[PPT_SMEM];
+        bool in_range[PPT_SMEM];
+        bool any_in = false;
+#pragma unroll
+        for (int k = 0; k < PPT_SMEM; k++) {
+            const long long pn = p0 + k * NT_SMEM + (long long)nseq * TILE;
+            xn[k] = (pn < n) ? __ldg(x + pn) : 1.0; qn[k] = (pn < n) ? __ldg(q2 + pn) : 1.0;
+            in_range[k] = (p0 + k * NT_SMEM < n) && xv[k] >= g.x_min && xv[k] <= g.x_max && qv[k] >= g.q2_min && qv[k] <= g.q2_max;
+            any_in |= in_range[k];
         }
-        const bool invalid = live && !in_range && (!(xv > 0.0) || !(qv > 0.0) || !(xv <= g.x_max) || isinf(qv));
-        const bool slow = live && !in_range && !invalid;
-        const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
-        if (invalid) {
-            store4(out, out_stride, p, row, false, make_double2(qnan, qnan), make_double2(qnan, qnan));
-            if (pass == 0) atomicAdd(g.n_invalid, 1ULL);
+        if (any_in) {
+            // ---- locate (LUT guess + exact comparisons where needed), weights, one gather per point.
+            // A lane whose point is out of range computes a dummy in-range point and stores nothing.
+            Win w[PPT_SMEM];
+            double vw[PPT_SMEM][4];
+#pragma unroll
+            for (int k = 0; k < PPT_SMEM; k++) {
+                const double xs = in_range[k] ? xv[k] : g.x_min, qs = in_range[k] ? qv[k] : g.q2_min;
+                const double u = ln_pos(xs), v = ln_pos(qs);
+                const int i = locate_x(g, sv, xs, u);
+                const int gi = locate_q(g, sv, qs, v);
+                const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
+                const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
+                double wu[4];
+                weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
+                weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vw[k]);
+                make_win(w[k], tab + (uint32_t)((gi - 1) * (int)RB), i - 1, wu, lane8);
+            }
+#pragma unroll
+            for (int k = 0; k < PPT_SMEM; k++) {
+                double2 E, O;
+                gather4(w[k], vw[k], rb1, rb2, rb3, E, O);
+                if (in_range[k]) store4(out, out_stride, p0 + k * NT_SMEM, row, odd, E, O);
+            }
         }
-        if (slow_mask) {  // warp-uniform: compact out-of-grid points into this warp's list
-            const int k = __popc(slow_mask);
-            if (wcount + k > 32) { flush(wcount); wcount = 0; }
-            if (slow) s_wlist[warp][wcount + __popc(slow_mask & ((1u << lane) - 1u))] = (it << 5) | (uint32_t)lane;
-            wcount += k;
+#pragma unroll
+        for (int k = 0; k < PPT_SMEM; k++) {
+            const long long p = p0 + k * NT_SMEM;
+            const bool live = p < n;
+            const bool invalid = live && !in_range[k] && (!(xv[k] > 0.0) || !(qv[k] > 0.0) || !(xv[k] <= g.x_max) || isinf(qv[k]));
+            const bool slow = live && !in_range[k] && !invalid;
+            const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
+            if (invalid) {
+                store4(out, out_stride, p, row, false, make_double2(qnan, qnan), make_double2(qnan, qnan));
+                if (pass == 0) atomicAdd(g.n_invalid, 1ULL);
+            }
+            if (slow_mask) {  // warp-uniform: compact out-of-grid points into this warp's list
+                const int c = __popc(slow_mask);
+                if (wcount + c > 32) { flush(wcount); wcount = 0; }
+                if (slow) s_wlist[warp][wcount + __popc(slow_mask & ((1u << lane) - 1u))] = ((it * PPT_SMEM + k) << 5) | (uint32_t)lane;
+                wcount += c;
+            }
+            xv[k] = xn[k]; qv[k] = qn[k];
         }
-        xv = xn; qv = qn;
     }
     if (wcount) flush(wcount);
 }
@@ -444,7 +474,7 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
     int per_pass = sms / pl.n;
     if (per_pass < 1) per_pass = 1;
-    long long tiles = (n + NT_SMEM - 1) / NT_SMEM;
+    long long tiles = (n + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
     if (per_pass > tiles) per_pass = (int)tiles;
     k_xfxq2_smem<<<per_pass * pl.n, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride);
     pdfb_count_launch(1);
