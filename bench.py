@@ -29,7 +29,7 @@ UNIT = "evaluations/s"
 N_FULL = 100_000_000
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_xfxq2_smem launch at 1e8 points x 11
 # flavours, from the `ncu --set full` capture summarised in profiles/r1_xfxq2_smem_full.md
-NCU_TRAFFIC_BYTES_PER_POINT = (1.641881e9 + 8.743990e9) / 1e8
+NCU_TRAFFIC_BYTES_PER_POINT = (1.650941e9 + 8.741799e9) / 1e8
 
 
 def measured_peaks():
@@ -222,6 +222,7 @@ def run_gpu(args):
     a1.record(); torch.cuda.synchronize()
     a_ms = a0.elapsed_time(a1) / 5
     peak, peak_src = measured_peaks()
+    sms = torch.cuda.get_device_properties(local).multi_processor_count
     bytes_per_launch = (16 + 8 * F) * n
     achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -238,8 +239,15 @@ def run_gpu(args):
                          "traffic_source": "profiles/r1_xfxq2_smem_full.md (ncu, 1e8 points; scaled by points)",
                          "kernel": "k_xfxq2_smem" if B.pdf_grid_uses_smem_path(h) else "k_xfxq2_v0", "kernel_ms": kern_ms,
                          "algorithmic_bytes_per_point": 16 + 8 * F, "peak_source": peak_src},
+            # the limit the kernel actually runs against: the per-point 4x4 stencil gather,
+            # 16 x 8 B x F of table per point through the SM's 128 B/clk shared-memory data pipe
+            "onchip_gather": {"bound": "smem", "achieved": 128 * F * n / (kern_ms * 1e-3) / 1e9,
+                              "peak": sms * 128 * (clocks["sm_mhz"] or 1965.0) * 1e6 / 1e9, "unit": "GB/s",
+                              "algorithmic_bytes_per_point": 128 * F,
+                              "note": "context only; the contract roofline is `roofline` (HBM)"},
             "alphas": {"points": n, "ms": a_ms, "evaluations_per_s": n / (a_ms * 1e-3),
                        "hbm_frac": 16 * n / (a_ms * 1e-3) / 1e9 / peak}}
+    line["onchip_gather"]["frac"] = line["onchip_gather"]["achieved"] / line["onchip_gather"]["peak"]
     B.alphas_grid_free(ha)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(grid, x_h, q2_h, pids)
