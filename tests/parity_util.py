@@ -19,8 +19,12 @@ def eq1_rel_diff(got, ref):
     return np.abs(got - ref) / (np.abs(ref) + EPS_EQ1)
 
 
-def check_parity(got, ref, scale=None, max_clause_frac=2e-3, what=""):
-    """Assert parity; returns a dict of statistics."""
+def check_parity(got, ref, scale=None, max_clause_frac=2e-3, what="", clause_rel=REL):
+    """Assert parity; returns a dict of statistics.
+
+    ``clause_rel`` widens the conditioning clause only (never the north_star rule) for grids whose
+    knots are much denser than the paper's: a last-bit difference in a coordinate logarithm moves
+    t by ulp(u)/dU, so the clause scales with |u|/dU; the caller derives the factor."""
     got, ref = np.asarray(got), np.asarray(ref)
     assert got.shape == ref.shape, (got.shape, ref.shape)
     nan_g, nan_r = np.isnan(got), np.isnan(ref)
@@ -37,7 +41,7 @@ def check_parity(got, ref, scale=None, max_clause_frac=2e-3, what=""):
         S = np.asarray(scale)[ok][~rule]
         worst = d[~rule] / S
         stats["max_d_over_S"] = float(worst.max())
-        bad = worst > REL
+        bad = worst > clause_rel
         assert not bad.any(), (f"{what}: {int(bad.sum())} outputs outside the conditioning clause, "
                                f"worst |d|/S = {worst.max():.3e}")
         assert n_clause <= max_clause_frac * max(1, ok.sum()), \

@@ -189,3 +189,47 @@ def test_tiny_subgrids_two_and_three_knots(torch_cuda):
     ref, sc = og.xfxq2([1, 21], x, q2, with_scale=True)
     check_parity(gpu_xfxq2(torch_cuda, h, [1, 21], x, q2), ref, sc, max_clause_frac=1.0, what="tiny")
     B.pdf_grid_free(h)
+
+
+def graded_knots(rng, lo, hi, n_regular, cluster, at):
+    """Knots on [lo, hi]: random ln-gaps with a cluster of small gaps spliced in at index `at`;
+    neighbouring gaps differ by at most ~4x (as in real grids), so derivative coefficients stay O(1)."""
+    gaps = list(rng.uniform(0.45, 1.0, n_regular))
+    gaps[at:at] = list(cluster)
+    gaps = np.asarray(gaps) * (np.log(hi / lo) / np.sum(gaps))
+    k = lo * np.exp(np.concatenate([[0.0], np.cumsum(gaps)]))
+    k[-1] = hi
+    return k
+
+
+def test_irregular_grid_on_the_smem_path(torch_cuda):
+    """Non-uniform knots with dense clusters (several knots per search-LUT bin), nx not a multiple
+    of 4, 4-knot sub-grids next to long ones, random values of both signs: every cell, knot and
+    threshold is scanned, plus out-of-grid points, for PID subsets that use 1, 2 and 3 flavour
+    groups, duplicates and PID 0.  The smallest gaps are 0.01 (ln Q^2) and 0.02 (ln x) against >= 0.09
+    in the paper-shaped grids: one ulp of u (|u| <= 16: 3.6e-15) moves t by up to 3.6e-13, and the
+    weights change by up to ~4 per unit t next to a 4x narrower neighbour, per axis, so the
+    conditioning clause is taken at 4e-12 * S here; the plain rule is unchanged."""
+    from test_oracle_pins import make_spec, rand_knots
+    rng = np.random.default_rng(77)
+    xk = graded_knots(rng, 1e-7, 1.0, 21, [0.25, 0.08, 0.025, 0.02, 0.02, 0.02, 0.025, 0.08, 0.25], 9)
+    assert len(xk) == 31 and len(xk) % 4 != 0
+    subs = [np.geomspace(1.3, 2.0, 4), graded_knots(rng, 2.0, 4.5, 8, [], 0), np.geomspace(4.5, 4.75, 4),
+            graded_knots(rng, 4.75, 3e3, 10, [0.15, 0.05, 0.018, 0.006, 0.006, 0.006, 0.018, 0.05, 0.15], 4)]
+    lutbin = np.log((3e3 / 1.3) ** 2) / 512
+    assert (np.diff(2 * np.log(subs[3])) < lutbin / 2).sum() >= 3      # several knots share a LUT bin
+    assert (np.diff(np.log(xk)) < np.log(1e7) / 512 / 1.2).sum() >= 3
+    pids_all = [-3, -2, -1, 1, 2, 3, 4, 21, 22]
+    values = [rng.normal(size=(len(xk), len(q), len(pids_all))) for q in subs]
+    spec = make_spec(xk, subs, pids_all, values=values)
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    h = B.load_pdf_spec(spec)
+    assert B.lib().pdf_grid_uses_smem_path(h) == 1
+    x, q2 = W.scan_points(spec, per_cell=3)
+    lo, hi = float(subs[0][0]) ** 2, float(subs[-1][-1]) ** 2
+    xo = np.exp(rng.uniform(np.log(1e-9), 0.0, 4000)); qo = np.exp(rng.uniform(np.log(lo / 4), np.log(hi * 4), 4000))
+    x, q2 = np.concatenate([x, xo]), np.concatenate([q2, qo])
+    for req in ([21], [0, 22], [4, -3, 1], pids_all, [2, 2, 21, -1, 3, 22, 2]):
+        ref, sc = og.xfxq2(req, x, q2, with_scale=True)
+        check_parity(gpu_xfxq2(torch_cuda, h, req, x, q2), ref, sc, max_clause_frac=1.0, what=f"irregular {req}", clause_rel=4e-12)
+    B.pdf_grid_free(h)
