@@ -64,7 +64,7 @@ class ClockSampler(threading.Thread):
                 for bit, name in names.items():
                     if r & bit:
                         self.reasons.add(name)
-                time.sleep(0.02)
+                time.sleep(0.002)
         except Exception as exc:  # NVML missing: report, do not fail the bench
             self.reasons.add(f"nvml_unavailable:{type(exc).__name__}")
 

@@ -79,6 +79,16 @@ int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long long n, const
               const double *q2, double *out, void *cuda_stream);
 
 /*
+ * pdf_xfxq -- the second interpolating method of the PDF ("interpolating methods
+ * (two for the PDF and two for alpha_s)"): the scale is given as Q in GeV.  Defined as
+ * pdf_xfxq2(x, Q*Q) with the product rounded once in fp64; Q <= 0 or NaN has no value (NaN,
+ * counted).  Same arguments, layout, ownership and errors as pdf_xfxq2.
+ *   q      device [n], fp64, Q in GeV
+ */
+int pdf_xfxq(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+             const double *q, double *out, void *cuda_stream);
+
+/*
  * pdf_xfxq2_host -- the same for HOST buffers (pinned or pageable): chunks are copied to the
  * device, evaluated and copied back on internal streams, overlapping the three stages.
  * Synchronous: returns when `out` is complete.  Staging buffers are owned by the handle.
@@ -118,6 +128,10 @@ int alphas_grid_load(int n_knots, const double *q_knots, const double *alphas, i
  */
 int alphas_q2(const pdfb_alphas *a, long long n, const double *q2, double *out,
               void *cuda_stream);
+
+/* alphas_q -- alpha_s at Q in GeV: alphas_q2(Q*Q), the product rounded once in
+ * fp64; Q <= 0 or NaN gives NaN.  q: device [n]; out: device [n]. */
+int alphas_q(const pdfb_alphas *a, long long n, const double *q, double *out, void *cuda_stream);
 
 /* alphas_q2 for HOST buffers; synchronous. */
 int alphas_q2_host(pdfb_alphas *a, long long n, const double *q2, double *out);

@@ -20,7 +20,7 @@ _ip = ctypes.POINTER(ctypes.c_int)
 _vp = ctypes.c_void_p
 _ll = ctypes.c_longlong
 
-EXPORTS = ("pdf_grid_load", "pdf_xfxq2", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
+EXPORTS = ("pdf_grid_load", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
            "pdfb_launch_count")
 
@@ -44,6 +44,10 @@ def lib():
                                     ctypes.c_int, ctypes.POINTER(_vp)]
         L.pdf_xfxq2.restype = ctypes.c_int
         L.pdf_xfxq2.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
+        L.pdf_xfxq.restype = ctypes.c_int
+        L.pdf_xfxq.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
+        L.alphas_q.restype = ctypes.c_int
+        L.alphas_q.argtypes = [_vp, _ll, _vp, _vp, _vp]
         L.pdf_xfxq2_host.restype = ctypes.c_int
         L.pdf_xfxq2_host.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp]
         L.pdf_grid_status.restype = ctypes.c_int
@@ -152,6 +156,15 @@ def pdf_xfxq2(g, pids, x, q2, out, stream=None, n=None):
     _check(rc, "pdf_xfxq2")
 
 
+def pdf_xfxq(g, pids, x, q, out, stream=None, n=None):
+    """Enqueue xf(x,Q), Q in GeV, for device tensors x, q -> out[n_req, n] on `stream`."""
+    pids = _i32(pids)
+    n = int(x.numel() if n is None else n)
+    rc = lib().pdf_xfxq(_vp(g), len(pids), pids.ctypes.data_as(_ip), n, _dev_ptr(x, n, "x"),
+                        _dev_ptr(q, n, "q"), _dev_ptr(out, len(pids) * n, "out"), _stream_ptr(stream))
+    _check(rc, "pdf_xfxq")
+
+
 def pdf_xfxq2_host(g, pids, x, q2, out):
     """Synchronous evaluation for HOST buffers (numpy or pinned torch CPU tensors)."""
     pids = _i32(pids)
@@ -194,6 +207,12 @@ def alphas_q2(a, q2, out, stream=None, n=None):
     n = int(q2.numel() if n is None else n)
     rc = lib().alphas_q2(_vp(a), n, _dev_ptr(q2, n, "q2"), _dev_ptr(out, n, "out"), _stream_ptr(stream))
     _check(rc, "alphas_q2")
+
+
+def alphas_q(a, q, out, stream=None, n=None):
+    n = int(q.numel() if n is None else n)
+    rc = lib().alphas_q(_vp(a), n, _dev_ptr(q, n, "q"), _dev_ptr(out, n, "out"), _stream_ptr(stream))
+    _check(rc, "alphas_q")
 
 
 def alphas_q2_host(a, q2, out):

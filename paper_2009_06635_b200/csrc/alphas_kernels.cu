@@ -7,7 +7,7 @@
 #define ALPHAS_SMEM_MAX_KNOTS 512
 
 __global__ void __launch_bounds__(256)
-k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__restrict__ out)
+k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__restrict__ out, int q_is_q)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     IntervalRec *rec = reinterpret_cast<IntervalRec *>(smem_raw);
@@ -21,6 +21,7 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < n; p += stride) {
         double qv = __ldcs(q2 + p);
+        if (q_is_q) qv = (qv > 0.0) ? qv * qv : -1.0;
         double res;
         if (!(qv > 0.0)) {
             res = __longlong_as_double(0x7ff8000000000000LL);
@@ -52,6 +53,7 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
 // one cubic in t per point.  Two points per thread keep two independent ln chains in flight.
 #define NT_ALPHAS 512
 
+template <bool Q_IS_Q>
 __global__ void __launch_bounds__(NT_ALPHAS, 2)
 k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__restrict__ q2,
               double *__restrict__ out)
@@ -66,6 +68,7 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
     auto eval = [&](double qv) -> double {
         double res;
+        if (Q_IS_Q) qv = (qv > 0.0) ? qv * qv : -1.0;  // Q in GeV -> Q^2
         if (qv >= A.q2_min && qv <= A.q2_max) {
             const double v = pdfb_ln(qv);
             int b = min(max((int)((v - A.lut_v0) * A.lut_inv_h), 0), PDFB_LUT_BINS - 1);
@@ -102,18 +105,20 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
     for (; p < n; p += stride) __stcs(out + p, eval(__ldcs(q2 + p)));
 }
 
-int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out, cudaStream_t st)
+int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out, cudaStream_t st, int q_is_q)
 {
     if (n == 0) return PDFB_OK;
     if (a->d.fast_ok) {
         static int attr_dev = -1;
         if (attr_dev != a->device) {
-            PDFB_CUDA(cudaFuncSetAttribute(k_alphas_fast, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
+            PDFB_CUDA(cudaFuncSetAttribute(k_alphas_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
+            PDFB_CUDA(cudaFuncSetAttribute(k_alphas_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
             attr_dev = a->device;
         }
         long long blocks = (n + NT_ALPHAS - 1) / NT_ALPHAS;
         if (blocks > 148 * 2) blocks = 148 * 2;
-        k_alphas_fast<<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
+        if (q_is_q) k_alphas_fast<true><<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
+        else k_alphas_fast<false><<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
         pdfb_count_launch(1);
         PDFB_CUDA(cudaGetLastError());
         return PDFB_OK;
@@ -121,7 +126,7 @@ int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, doub
     size_t smem = (size_t)a->d.K * (sizeof(IntervalRec) + 16);
     long long blocks = (n + 255) / 256;
     if (blocks > 148 * 8) blocks = 148 * 8;
-    k_alphas<<<(unsigned)blocks, 256, smem, st>>>(a->d, n, q2, out);
+    k_alphas<<<(unsigned)blocks, 256, smem, st>>>(a->d, n, q2, out, q_is_q);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

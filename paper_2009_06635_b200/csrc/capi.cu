@@ -243,6 +243,17 @@ extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long lo
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream);
 }
 
+extern "C" int pdf_xfxq(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                        const double *q, double *out, void *cuda_stream)
+{
+    if (!g || !pids || n < 0) return PDFB_EINVAL;
+    if (n > 0 && (!x || !q || !out)) return PDFB_EINVAL;
+    int cols[PDFB_MAX_PIDS];
+    int rc = resolve_cols(g, n_req, pids, cols);
+    if (rc) return rc;
+    return pdfb_launch_xfxq2(g, n_req, cols, n, x, q, out, n, (cudaStream_t)cuda_stream, 1);
+}
+
 extern "C" int pdf_grid_uses_smem_path(const pdfb_grid *g) { return g ? g->d.smem_ok : 0; }
 
 extern "C" int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points)

@@ -92,6 +92,13 @@ extern "C" int alphas_q2(const pdfb_alphas *a, long long n, const double *q2, do
     return pdfb_launch_alphas(a, n, q2, out, (cudaStream_t)cuda_stream);
 }
 
+extern "C" int alphas_q(const pdfb_alphas *a, long long n, const double *q, double *out, void *cuda_stream)
+{
+    if (!a || n < 0) return PDFB_EINVAL;
+    if (n > 0 && (!q || !out)) return PDFB_EINVAL;
+    return pdfb_launch_alphas(a, n, q, out, (cudaStream_t)cuda_stream, 1);
+}
+
 extern "C" void alphas_grid_free(pdfb_alphas *a)
 {
     if (!a) return;

@@ -183,17 +183,18 @@ void pdfb_fill_lut(unsigned short *lut, const double *Z, const double *R, int nk
 void pdfb_count_launch(int n);
 
 // kernels' host launchers
+// q_is_q != 0: the scale array holds Q in GeV, not Q^2; the kernels square it once on load
 int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                      const double *q2, double *out, long long out_stride, cudaStream_t st);
+                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q = 0);
 int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out,
-                       cudaStream_t st);
+                       cudaStream_t st, int q_is_q = 0);
 int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_rec32, int n_arrays,
                        const int *h_off, cudaStream_t st);
 int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
                             int n_pid, int n_groups, long long group_stride, cudaStream_t st);
 int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st);
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q);
 int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st);
 int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, unsigned char *d_lines, int n_sub,
                             const int *h_off, cudaStream_t st);

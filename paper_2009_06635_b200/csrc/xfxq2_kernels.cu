@@ -80,11 +80,12 @@ __device__ __forceinline__ double contract(const double *__restrict__ val, int k
 
 __global__ void __launch_bounds__(256)
 k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, const double *__restrict__ q2,
-           double *__restrict__ out, long long out_stride)
+           double *__restrict__ out, long long out_stride, int q_is_q)
 {
     long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (p >= n) return;
     double xv = x[p], qv = q2[p];
+    if (q_is_q) qv = (qv > 0.0) ? qv * qv : -1.0;  // Q in GeV -> Q^2 (a non-positive Q is invalid)
     if (!(xv > 0.0) || !(qv > 0.0) || !(xv <= g.x_max) || isinf(qv)) {
         for (int r = 0; r < rc.n; r++) out[r * out_stride + p] = __longlong_as_double(0x7ff8000000000000LL);
         atomicAdd(g.n_invalid, 1ULL);
@@ -159,15 +160,15 @@ k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, con
 }
 
 int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                      const double *q2, double *out, long long out_stride, cudaStream_t st)
+                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q)
 {
     if (n == 0) return PDFB_OK;
-    if (g->d.smem_ok) return pdfb_launch_xfxq2_smem(g, n_req, cols, n, x, q2, out, out_stride, st);
+    if (g->d.smem_ok) return pdfb_launch_xfxq2_smem(g, n_req, cols, n, x, q2, out, out_stride, st, q_is_q);
     ReqCols rc;
     rc.n = n_req;
     for (int r = 0; r < n_req; r++) rc.col[r] = cols[r];
     long long blocks = (n + 255) / 256;
-    k_xfxq2_v0<<<(unsigned)blocks, 256, 0, st>>>(g->d, rc, n, x, q2, out, out_stride);
+    k_xfxq2_v0<<<(unsigned)blocks, 256, 0, st>>>(g->d, rc, n, x, q2, out, out_stride, q_is_q);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

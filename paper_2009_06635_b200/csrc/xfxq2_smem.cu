@@ -295,6 +295,15 @@ __device__ __forceinline__ void store4(double *__restrict__ out, long long out_s
     if (row[3] >= 0) __stcs(out + row[3] * out_stride + p, c3);
 }
 
+// the scale of a point: Q^2, or Q in GeV squared once on load (a non-positive Q is invalid, like Q^2 <= 0)
+template <bool Q_IS_Q>
+__device__ __forceinline__ double load_scale(const double *p)
+{
+    const double q = __ldg(p);
+    return Q_IS_Q ? ((q > 0.0) ? q * q : -1.0) : q;
+}
+
+template <bool Q_IS_Q>  // compile-time: a run-time flag costs 11 % (register pressure at the 128 cap)
 __global__ void __launch_bounds__(NT_SMEM, 1)
 k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
              const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
@@ -355,7 +364,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const uint32_t ik = e >> 5;
             const long long ps = ((long long)seq + (long long)(ik / PPT_SMEM) * nseq) * TILE + (ik % PPT_SMEM) * NT_SMEM +
                                  warp * 32 + (e & 31);
-            const Y4 r = slow_point(&g, smem, __ldg(x + ps), __ldg(q2 + ps), lane8);
+            const Y4 r = slow_point(&g, smem, __ldg(x + ps), load_scale<Q_IS_Q>(q2 + ps), lane8);
             store4(out, out_stride, ps, row, odd, r.E, r.O);  // the gather ran on THIS lane: its parity
         }
         __syncwarp();
@@ -367,7 +376,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 #pragma unroll
     for (int k = 0; k < PPT_SMEM; k++) {
         const long long p = tile * TILE + k * NT_SMEM + tid;
-        xv[k] = (p < n) ? __ldg(x + p) : 1.0; qv[k] = (p < n) ? __ldg(q2 + p) : 1.0;
+        xv[k] = (p < n) ? __ldg(x + p) : 1.0; qv[k] = (p < n) ? load_scale<Q_IS_Q>(q2 + p) : 1.0;
     }
     for (uint32_t it = 0; tile * TILE < n; tile += nseq, ++it) {
         const long long p0 = tile * TILE + tid;
@@ -377,7 +386,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 #pragma unroll
         for (int k = 0; k < PPT_SMEM; k++) {
             const long long pn = p0 + k * NT_SMEM + (long long)nseq * TILE;
-            xn[k] = (pn < n) ? __ldg(x + pn) : 1.0; qn[k] = (pn < n) ? __ldg(q2 + pn) : 1.0;
+            xn[k] = (pn < n) ? __ldg(x + pn) : 1.0; qn[k] = (pn < n) ? load_scale<Q_IS_Q>(q2 + pn) : 1.0;
             in_range[k] = (p0 + k * NT_SMEM < n) && xv[k] >= g.x_min && xv[k] <= g.x_max && qv[k] >= g.q2_min && qv[k] <= g.q2_max;
             any_in |= in_range[k];
         }
@@ -441,7 +450,8 @@ int pdfb_smem_eligible(const pdfb_grid *g)
     // the attribute is per function, not per handle: raise it once to the device maximum
     static int attr_set_for = -1;
     if (attr_set_for != g->device) {
-        if (cudaFuncSetAttribute(k_xfxq2_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - STATIC_SMEM) != cudaSuccess) {
+        if (cudaFuncSetAttribute(k_xfxq2_smem<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - STATIC_SMEM) != cudaSuccess ||
+            cudaFuncSetAttribute(k_xfxq2_smem<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - STATIC_SMEM) != cudaSuccess) {
             cudaGetLastError();
             return 0;
         }
@@ -451,7 +461,7 @@ int pdfb_smem_eligible(const pdfb_grid *g)
 }
 
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st)
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q)
 {
     // passes: one per (flavour group, distinct use of its columns); duplicates get extra passes
     PassList pl;
@@ -476,7 +486,10 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     if (per_pass < 1) per_pass = 1;
     long long tiles = (n + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
     if (per_pass > tiles) per_pass = (int)tiles;
-    k_xfxq2_smem<<<per_pass * pl.n, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride);
+    if (q_is_q)
+        k_xfxq2_smem<true><<<per_pass * pl.n, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride);
+    else
+        k_xfxq2_smem<false><<<per_pass * pl.n, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

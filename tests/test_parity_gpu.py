@@ -233,3 +233,46 @@ def test_irregular_grid_on_the_smem_path(torch_cuda):
         ref, sc = og.xfxq2(req, x, q2, with_scale=True)
         check_parity(gpu_xfxq2(torch_cuda, h, req, x, q2), ref, sc, max_clause_frac=1.0, what=f"irregular {req}", clause_rel=4e-12)
     B.pdf_grid_free(h)
+
+
+def test_q_argument_entry_points(torch_cuda, grid2, ograph2, h2):
+    """pdf_xfxq / alphas_q (the second interpolating method of each quantity) are
+    defined as the Q^2 methods at Q*Q rounded once: bit-identical to pdf_xfxq2 / alphas_q2 on the
+    squared scales of the same batch, and within tolerance of the oracle at those scales; Q <= 0 and
+    NaN give NaN and are counted."""
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    x, q2 = W.queries_extrapolation_mix(grid2, 60_001)
+    q = np.sqrt(q2)
+    qq = q * q
+    dx, dq, dqq = (torch.from_numpy(a).cuda() for a in (x, q, qq))
+    out_q = torch.empty((len(pids), len(x)), dtype=torch.float64, device="cuda")
+    out_q2 = torch.empty_like(out_q)
+    B.pdf_xfxq(h2, pids, dx, dq, out_q)
+    B.pdf_xfxq2(h2, pids, dx, dqq, out_q2)
+    torch.cuda.synchronize()
+    a, b = out_q.cpu().numpy(), out_q2.cpu().numpy()
+    assert np.array_equal(a, b, equal_nan=True)
+    ref, sc = ograph2.xfxq2(pids, x, qq, with_scale=True)
+    check_parity(a, ref, sc, max_clause_frac=5e-3, what="xfxq")
+    # no value for Q <= 0, NaN
+    before = B.pdf_grid_status(h2)
+    bx = torch.tensor([0.1, 0.1, 0.1, 0.1], dtype=torch.float64, device="cuda")
+    bq = torch.tensor([0.0, -2.0, float("nan"), 10.0], dtype=torch.float64, device="cuda")
+    bo = torch.empty((len(pids), 4), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq(h2, pids, bx, bq, bo)
+    bo = bo.cpu().numpy()
+    assert np.isnan(bo[:, :3]).all() and np.isfinite(bo[:, 3]).all()
+    assert B.pdf_grid_status(h2) - before == 3
+    aspec = W.make_alphas_grid()
+    ha = B.load_alphas_spec(aspec)
+    ra, rb, rc = torch.empty_like(dq), torch.empty_like(dq), torch.empty_like(bq)
+    B.alphas_q(ha, dq, ra)
+    B.alphas_q2(ha, dqq, rb)
+    B.alphas_q(ha, bq, rc)
+    torch.cuda.synchronize()
+    ra, rb, rc = ra.cpu().numpy(), rb.cpu().numpy(), rc.cpu().numpy()
+    assert np.array_equal(ra, rb)
+    assert np.isnan(rc[:3]).all() and np.isfinite(rc[3])
+    check_parity(ra, oracle.OracleAlphas.from_spec(aspec).q2(qq), what="alphas_q")
+    B.alphas_grid_free(ha)
