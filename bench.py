@@ -247,7 +247,16 @@ def run_gpu(args):
                               "note": "context only; the contract roofline is `roofline` (HBM)"},
             "alphas": {"points": n, "ms": a_ms, "evaluations_per_s": n / (a_ms * 1e-3),
                        "hbm_frac": 16 * n / (a_ms * 1e-3) / 1e9 / peak}}
-    line["onchip_gather"]["frac"] = line["onchip_gather"]["achieved"] / line["onchip_gather"]["peak"]
+    # measured denominators for the two bounds MEASURED_PEAKS.json does not carry (pdfb_probe)
+    lds_bps, fma_ps = B.probe(B.PROBE_LDS, local), B.probe(B.PROBE_FP64, local)
+    og = line["onchip_gather"]
+    og["peak_nominal"], og["peak"], og["peak_source"] = og["peak"], lds_bps / 1e9, "measured: pdfb_probe(PDFB_PROBE_LDS), conflict-free LDS.128"
+    og["frac"] = og["achieved"] / og["peak"]
+    w_f = 2 * 28 + 32 + 16 + 16 * F  # algorithmic FP64-pipe operations per in-range point, SURVEY.md 8(d)
+    line["fp64"] = {"bound": "alu", "achieved": w_f * n / (kern_ms * 1e-3) / 1e12, "peak": fma_ps / 1e12,
+                    "unit": "T FP64 op/s (FMA = 1)", "frac": w_f * n / (kern_ms * 1e-3) / fma_ps,
+                    "algorithmic_ops_per_point": w_f, "peak_source": "measured: pdfb_probe(PDFB_PROBE_FP64), DFMA chains",
+                    "note": "context only; HBM is the slower of the two contract bounds"}
     B.alphas_grid_free(ha)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(grid, x_h, q2_h, pids)

@@ -147,6 +147,18 @@ int pdfb_debug_ln(const double *in, double *out, long long n, void *cuda_stream)
 /* Kernels launched by this library since load (all handles); for bench accounting. */
 long long pdfb_launch_count(void);
 
+/*
+ * pdfb_probe -- machine probes for the bounds MEASURED_PEAKS.json does not carry (SURVEY.md 8(d):
+ * the FP64 peak must be measured).  Not part of the method; used by bench.py only.
+ *   PDFB_PROBE_FP64  *result = FP64 fused multiply-adds per second (thread level) of independent
+ *                    DFMA chains at full occupancy
+ *   PDFB_PROBE_LDS   *result = bytes per second delivered by conflict-free LDS.128 from shared memory
+ * Synchronous; allocates and frees its own scratch.  result: host pointer.
+ */
+#define PDFB_PROBE_FP64 1
+#define PDFB_PROBE_LDS 2
+int pdfb_probe(int which, int device, double *result);
+
 #ifdef __cplusplus
 }
 #endif

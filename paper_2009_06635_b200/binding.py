@@ -22,7 +22,7 @@ _ll = ctypes.c_longlong
 
 EXPORTS = ("pdf_grid_load", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
-           "pdfb_launch_count")
+           "pdfb_launch_count", "pdfb_probe")
 
 
 class PdfbError(RuntimeError):
@@ -69,6 +69,8 @@ def lib():
         L.pdfb_strerror.restype = ctypes.c_char_p
         L.pdfb_strerror.argtypes = [ctypes.c_int]
         L.pdfb_launch_count.restype = _ll
+        L.pdfb_probe.restype = ctypes.c_int
+        L.pdfb_probe.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
         L.pdfb_debug_ln.restype = ctypes.c_int
         L.pdfb_debug_ln.argtypes = [_vp, _vp, _ll, _vp]
         _lib = L
@@ -81,6 +83,16 @@ def strerror(code: int) -> str:
 
 def launch_count() -> int:
     return int(lib().pdfb_launch_count())
+
+
+PROBE_FP64, PROBE_LDS = 1, 2
+
+
+def probe(which: int, device: int = 0) -> float:
+    """Machine probe (pdfb200.h): FP64 FMA/s or shared-memory bytes/s."""
+    r = ctypes.c_double(0.0)
+    _check(lib().pdfb_probe(int(which), int(device), ctypes.byref(r)), "pdfb_probe")
+    return float(r.value)
 
 
 def debug_ln(x, out, stream=None):
