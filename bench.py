@@ -121,6 +121,35 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def bench_members(torch, B, local, n_rep):
+    """SURVEY.md 8(f).1 / PAPER.md:171-190, Table 2: all 13 flavours of N_rep members on a 2415-point
+    x-grid, one pdf_xfxq2_members launch; reported beside the metric, not inside it."""
+    g0 = W.grid_member(0)
+    vals = W.member_values(n_rep)
+    hs = B.pdf_set_load(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals, device=local)
+    pids = list(W.PIDS_13)
+    x, q2 = W.queries_fk_xgrid(g0)
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    out = torch.empty((n_rep, len(pids), len(x)), dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        B.pdf_xfxq2_members(hs, 0, n_rep, pids, dx, dq, out)
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(10):
+        B.pdf_xfxq2_members(hs, 0, n_rep, pids, dx, dq, out)
+    b.record(); torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / 10
+    B.pdf_grid_free(hs)
+    ev = n_rep * len(pids) * len(x)
+    # the slices are read once from HBM (the set does not fit L2 at N_rep = 400), the outputs written once
+    bytes_alg = n_rep * 4 * 100 * 64 * 32 + 8 * ev
+    paper = {10: 0.07, 50: 0.35, 100: 0.69, 200: 1.46, 300: 1.29, 400: 1.69}.get(n_rep)
+    return {"n_rep": n_rep, "flavours": len(pids), "points": len(x), "ms": ms, "evaluations_per_s": ev / (ms * 1e-3),
+            "algorithmic_bytes": bytes_alg, "hbm_gbs": bytes_alg / (ms * 1e-3) / 1e9,
+            "paper_pdfflow_gpu_s": paper, "paper_hardware": "system P1 (Titan V / RTX 2080 Ti), PAPER.md:179-188: context, another machine",
+            "workload": "synthetic member tables on the NNPDF-shaped knots (workloads.member_values)"}
+
+
 def run_gpu(args):
     import torch
     from paper_2009_06635_b200 import binding as B, build
@@ -258,6 +287,8 @@ def run_gpu(args):
                     "algorithmic_ops_per_point": w_f, "peak_source": "measured: pdfb_probe(PDFB_PROBE_FP64), DFMA chains",
                     "note": "context only; HBM is the slower of the two contract bounds"}
     B.alphas_grid_free(ha)
+    if not args.no_members:
+        line["multi_member"] = bench_members(torch, B, local, args.members)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(grid, x_h, q2_h, pids)
     B.pdf_grid_free(h)
@@ -277,6 +308,8 @@ def main():
     ap.add_argument("--ref-points", type=int, default=2_000_000, help="oracle sample per step")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-members", action="store_true")
+    ap.add_argument("--members", type=int, default=400, help="N_rep of the multi-member leg (Table 2)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -42,6 +42,7 @@ enum {
 };
 #define PDFB_MAX_SUBGRIDS 16
 #define PDFB_MAX_PIDS 32
+#define PDFB_MAX_MEMBERS 4096
 
 /*
  * pdf_grid_load -- upload one PDF member's knot grid and run the grid-setup kernel
@@ -64,6 +65,31 @@ enum {
 int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
                   const double *q_knots, int n_pid, const int *pids, const double *values,
                   int device, pdfb_grid **out);
+
+/*
+ * pdf_set_load -- a PDF SET: n_members member tables on the same knots (section
+ * 4.3 "Multi-PDF members evaluation": all flavours of N_rep members on one batch of points).
+ * Arguments as pdf_grid_load, plus
+ *   n_members  1 .. PDFB_MAX_MEMBERS
+ *   values     host, [member][s][ix][iq][ipid]: each member in LHAPDF grid-file order
+ * pdf_grid_load is pdf_set_load with one member; pdf_xfxq2 / pdf_xfxq evaluate member 0.
+ */
+int pdf_set_load(int n_members, int n_sub, int nx, const double *x_knots, const int *q_offsets,
+                 const double *q_knots, int n_pid, const int *pids, const double *values,
+                 int device, pdfb_grid **out);
+
+/* Number of members of the handle (0 on NULL). */
+int pdf_set_members(const pdfb_grid *g);
+
+/*
+ * pdf_xfxq2_members -- members member0 .. member0+n_mem-1 on the SAME n points: every member is
+ * the interpolation of pdf_xfxq2 applied to its own table (cell location and weights do not depend
+ * on the member).  One launch; allocates nothing, never synchronises.
+ *   out    device [n_mem][n_req][n]: out[(m*n_req + r)*n + p] = xf of pids[r], member member0+m, point p
+ * PDFB_EINVAL if the member range is not inside the set.  Points with no value are counted once.
+ */
+int pdf_xfxq2_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
+                      long long n, const double *x, const double *q2, double *out, void *cuda_stream);
 
 /*
  * pdf_xfxq2 -- xf_pid(x, Q^2) for n points and n_req flavours (section 2.2;

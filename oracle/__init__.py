@@ -141,3 +141,20 @@ class OracleAlphas:
         if getattr(self, "_h", None) and _lib is not None:
             _lib.oracle_alphas_free(self._h)
             self._h = None
+
+
+def xfxq2_members(x_knots, q_offsets, q_knots, grid_pids, member_values, pids, x, q2, with_scale: bool = False):
+    """A PDF set (section 4.3): member m is the single-member interpolation applied
+    to member_values[m] on the shared knots -- the definition written out, one member at a time.
+    Returns [n_members, n_req, n] (and the scale array of the same shape)."""
+    outs, scales = [], []
+    for vals in member_values:
+        og = OraclePdfGrid(x_knots, q_offsets, q_knots, grid_pids, vals)
+        r = og.xfxq2(pids, x, q2, with_scale=with_scale)
+        if with_scale:
+            outs.append(r[0]); scales.append(r[1])
+        else:
+            outs.append(r)
+    if with_scale:
+        return np.stack(outs), np.stack(scales)
+    return np.stack(outs)

@@ -20,7 +20,7 @@ _ip = ctypes.POINTER(ctypes.c_int)
 _vp = ctypes.c_void_p
 _ll = ctypes.c_longlong
 
-EXPORTS = ("pdf_grid_load", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
+EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
            "pdfb_launch_count", "pdfb_probe")
 
@@ -42,6 +42,13 @@ def lib():
         L.pdf_grid_load.restype = ctypes.c_int
         L.pdf_grid_load.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _ip, _dp, ctypes.c_int, _ip, _dp,
                                     ctypes.c_int, ctypes.POINTER(_vp)]
+        L.pdf_set_load.restype = ctypes.c_int
+        L.pdf_set_load.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, _ip, _dp, ctypes.c_int, _ip, _dp,
+                                   ctypes.c_int, ctypes.POINTER(_vp)]
+        L.pdf_set_members.restype = ctypes.c_int
+        L.pdf_set_members.argtypes = [_vp]
+        L.pdf_xfxq2_members.restype = ctypes.c_int
+        L.pdf_xfxq2_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq2.restype = ctypes.c_int
         L.pdf_xfxq2.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq.restype = ctypes.c_int
@@ -157,6 +164,35 @@ def pdf_grid_load(x_knots, q_offsets, q_knots, pids, values, device: int = 0):
                              ctypes.byref(h))
     _check(rc, "pdf_grid_load")
     return h.value
+
+
+def pdf_set_load(x_knots, q_offsets, q_knots, pids, values, device: int = 0):
+    """-> handle of a PDF set; values[member] = one member's table in LHAPDF grid-file order."""
+    x_knots, q_knots = _f64(x_knots), _f64(q_knots)
+    q_offsets, pids = _i32(q_offsets), _i32(pids)
+    values = _f64(values)
+    if values.ndim != 2:
+        raise ValueError("values must be [n_members, table size]")
+    h = _vp()
+    rc = lib().pdf_set_load(values.shape[0], len(q_offsets) - 1, len(x_knots), x_knots.ctypes.data_as(_dp),
+                            q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
+                            pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp), int(device), ctypes.byref(h))
+    _check(rc, "pdf_set_load")
+    return h.value
+
+
+def pdf_set_members(g) -> int:
+    return int(lib().pdf_set_members(_vp(g)))
+
+
+def pdf_xfxq2_members(g, member0, n_mem, pids, x, q2, out, stream=None, n=None):
+    """Enqueue members member0..member0+n_mem-1 on the same points -> out[n_mem, n_req, n]."""
+    pids = _i32(pids)
+    n = int(x.numel() if n is None else n)
+    rc = lib().pdf_xfxq2_members(_vp(g), int(member0), int(n_mem), len(pids), pids.ctypes.data_as(_ip), n,
+                                 _dev_ptr(x, n, "x"), _dev_ptr(q2, n, "q2"),
+                                 _dev_ptr(out, int(n_mem) * len(pids) * n, "out"), _stream_ptr(stream))
+    _check(rc, "pdf_xfxq2_members")
 
 
 def pdf_xfxq2(g, pids, x, q2, out, stream=None, n=None):

@@ -51,10 +51,11 @@ void pdfb_fill_lut(unsigned short *lut, const double *Z, const double *R, int nk
 }
 
 // ------------------------------------------------------------------------------ PDF grid
-extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
-                             const double *q_knots, int n_pid, const int *pids, const double *values,
-                             int device, pdfb_grid **out)
+extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_knots, const int *q_offsets,
+                            const double *q_knots, int n_pid, const int *pids, const double *values,
+                            int device, pdfb_grid **out)
 {
+    if (n_members < 1 || n_members > PDFB_MAX_MEMBERS) return out ? (*out = nullptr, PDFB_ELIMIT) : PDFB_EINVAL;
     if (!out) return PDFB_EINVAL;
     *out = nullptr;
     if (!x_knots || !q_offsets || !q_knots || !pids || !values) return PDFB_EINVAL;
@@ -84,7 +85,7 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     memset(g, 0, sizeof(*g));
     g->device = device;
     GridDev &d = g->d;
-    d.n_sub = n_sub; d.nx = nx; d.n_pid = n_pid; d.nq_tot = nq_tot;
+    d.n_sub = n_sub; d.nx = nx; d.n_pid = n_pid; d.nq_tot = nq_tot; d.n_members = n_members;
     d.kpad = (n_pid + 1) & ~1;  // even number of doubles per knot: 16-byte aligned knots
     memcpy(g->pids, pids, sizeof(int) * n_pid);
 
@@ -112,7 +113,8 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     size_t o_xrec = align_up(o_z + sizeof(double) * (nx + nq_tot + 1), 128);
     size_t o_qrec = align_up(o_xrec + sizeof(IntervalRec) * nx, 128);
     size_t o_val = align_up(o_qrec + sizeof(IntervalRec) * nq_tot, 128);
-    size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad, 128);
+    d.val_mstride = knots * d.kpad;  // one member's table, in doubles
+    size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad * n_members, 128);
     size_t o_raw = align_up(o_cnt + 128, 128);
     // shared-memory path: flavour-group slices and the aux block
     d.nx4 = (nx + 3) & ~3;
@@ -132,8 +134,8 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     d.post_bytes = (int)align_up((size_t)std::max(128 * nq_tot, d.nx4 * 32 + 128), 128);
     if (128 * nx < d.nx4 * 32 + 32) d.smem_ok = 0;  // (never: 128 nx >= 32 nx4 + 32 for nx >= 2)
     const int aux_bytes = d.pre_bytes + d.post_bytes;
-    size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid, 128);
-    size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups, 128);
+    size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid * n_members, 128);
+    size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_members, 128);
     size_t total = o_aux + aux_bytes;
     char *blob = nullptr;
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
@@ -145,7 +147,7 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
     do {
         if (cudaMemcpy(blob + o_xk, x_knots, sizeof(double) * nx, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(blob + o_q2k, h_q2.data(), sizeof(double) * (nq_tot + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(blob + o_raw, values, sizeof(double) * knots * n_pid, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(blob + o_raw, values, sizeof(double) * knots * n_pid * n_members, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemset(blob + o_cnt, 0, 128) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         cudaEventRecord(e0, 0);
         // K1: ln of the knots (and of rule C's probe scale), read back for the host-side tables
@@ -176,16 +178,20 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
         rc = pdfb_setup_records((const double *)(blob + o_z) + nx, (IntervalRec *)(blob + o_qrec),
                                 (IntervalRec32 *)(blob + o_aux + d.pre_bytes + d.a_qrec), n_sub, d.q_off, 0);
         if (rc) break;
-        // K1: value table re-layout, sub-grid by sub-grid
+        // K1: value table re-layout, member by member, sub-grid by sub-grid
         long long src = 0;
-        for (int s = 0; s < n_sub && !rc; s++) {
-            int nq = q_offsets[s + 1] - q_offsets[s];
-            rc = pdfb_setup_values((const double *)(blob + o_raw) + src,
-                                   (double *)(blob + o_val) + (long long)d.v_off[s] * d.kpad, nx, nq, n_pid, d.kpad, 0);
-            if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src, (double *)(blob + o_valg),
-                                                  q_offsets[s] * d.nx4, nx, d.nx4, nq, n_pid, d.n_groups,
-                                                  (long long)d.slice_bytes / 8, 0);
-            src += (long long)nx * nq * n_pid;
+        for (int m = 0; m < n_members && !rc; m++) {
+            double *valg_m = (double *)(blob + o_valg) + (long long)m * d.n_groups * (d.slice_bytes / 8);
+            for (int s = 0; s < n_sub && !rc; s++) {
+                int nq = q_offsets[s + 1] - q_offsets[s];
+                rc = pdfb_setup_values((const double *)(blob + o_raw) + src,
+                                       (double *)(blob + o_val) + m * d.val_mstride + (long long)d.v_off[s] * d.kpad,
+                                       nx, nq, n_pid, d.kpad, 0);
+                if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src, valg_m,
+                                                      q_offsets[s] * d.nx4, nx, d.nx4, nq, n_pid, d.n_groups,
+                                                      (long long)d.slice_bytes / 8, 0);
+                src += (long long)nx * nq * n_pid;
+            }
         }
         if (rc) break;
         cudaEventRecord(e1, 0);
@@ -230,6 +236,28 @@ static int resolve_cols(const pdfb_grid *g, int n_req, const int *pids, int *col
         if (cols[r] < 0) return PDFB_EPID;
     }
     return PDFB_OK;
+}
+
+extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
+                             const double *q_knots, int n_pid, const int *pids, const double *values,
+                             int device, pdfb_grid **out)
+{
+    return pdf_set_load(1, n_sub, nx, x_knots, q_offsets, q_knots, n_pid, pids, values, device, out);
+}
+
+extern "C" int pdf_set_members(const pdfb_grid *g) { return g ? g->d.n_members : 0; }
+
+extern "C" int pdf_xfxq2_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
+                                 long long n, const double *x, const double *q2, double *out, void *cuda_stream)
+{
+    if (!g || !pids || n < 0 || n_mem < 0) return PDFB_EINVAL;
+    if (member0 < 0 || member0 + n_mem > g->d.n_members) return PDFB_EINVAL;
+    if (n > 0 && n_mem > 0 && (!x || !q2 || !out)) return PDFB_EINVAL;
+    int cols[PDFB_MAX_PIDS];
+    int rc = resolve_cols(g, n_req, pids, cols);
+    if (rc) return rc;
+    if (n_mem == 0) return PDFB_OK;
+    return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream, 0, member0, n_mem);
 }
 
 extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,

@@ -91,6 +91,8 @@ __device__ __forceinline__ double pdfb_ln(double a)
 
 struct GridDev {
     int n_sub, nx, n_pid, nq_tot;
+    int n_members;                     // member tables sharing these knots (pdf_set_load)
+    long long val_mstride;             // doubles between two members in `val`
     int kpad;                          // doubles per knot in `val` (>= n_pid)
     int q_off[PDFB_MAX_SUBGRIDS + 1];  // knot offsets of the sub-grids
     int v_off[PDFB_MAX_SUBGRIDS];      // offset (in knots) of sub-grid s in `val`
@@ -105,13 +107,13 @@ struct GridDev {
     const double *q2k;                 // [nq_tot] Q^2 knots
     const IntervalRec *xrec;           // [nx-1]
     const IntervalRec *qrec;           // [nq_tot]; entry q_off[s]+j = interval j of sub-grid s
-    const double *val;                 // [s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
+    const double *val;                 // [member][s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
     unsigned long long *n_invalid;     // sticky counter
     // ---- shared-memory path (xfxq2_smem.cu): flavour-group slices + a small aux block
     int smem_ok;                       // 1 if the grid qualifies (nx >= 4, every sub-grid >= 4 Q knots)
     int n_groups, nx4;                 // groups of 4 value columns; nx padded to a multiple of 4
     int slice_bytes;                   // one group's slice: nq_tot * nx4 * 32 B
-    const double *valg;                // [group][s][iq][ix4][4]
+    const double *valg;                // [member][group][s][iq][ix4][4]
     const unsigned char *aux;          // [pre | post] blocks, copied verbatim around the slice
     int pre_bytes, post_bytes;         // shared memory = [pre | slice | post]
     int a_xk, a_q2k, a_lutx, a_lutq, a_xrec;  // byte offsets inside pre (a_xrec is its tail)
@@ -185,7 +187,8 @@ void pdfb_count_launch(int n);
 // kernels' host launchers
 // q_is_q != 0: the scale array holds Q in GeV, not Q^2; the kernels square it once on load
 int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q = 0);
+                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q = 0,
+                      int member0 = 0, int n_mem = 1);
 int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out,
                        cudaStream_t st, int q_is_q = 0);
 int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_rec32, int n_arrays,
@@ -194,7 +197,8 @@ int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off,
                             int n_pid, int n_groups, long long group_stride, cudaStream_t st);
 int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q);
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
+                           int member0, int n_mem);
 int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st);
 int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, unsigned char *d_lines, int n_sub,
                             const int *h_off, cudaStream_t st);

@@ -80,15 +80,18 @@ __device__ __forceinline__ double contract(const double *__restrict__ val, int k
 
 __global__ void __launch_bounds__(256)
 k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, const double *__restrict__ q2,
-           double *__restrict__ out, long long out_stride, int q_is_q)
+           double *__restrict__ out, long long out_stride, int q_is_q, int member0)
 {
     long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (p >= n) return;
+    // blockIdx.y = member of the set: its table, and its block of rc.n output rows
+    g.val += (long long)(member0 + blockIdx.y) * g.val_mstride;
+    out += (long long)blockIdx.y * rc.n * out_stride;
     double xv = x[p], qv = q2[p];
     if (q_is_q) qv = (qv > 0.0) ? qv * qv : -1.0;  // Q in GeV -> Q^2 (a non-positive Q is invalid)
     if (!(xv > 0.0) || !(qv > 0.0) || !(xv <= g.x_max) || isinf(qv)) {
         for (int r = 0; r < rc.n; r++) out[r * out_stride + p] = __longlong_as_double(0x7ff8000000000000LL);
-        atomicAdd(g.n_invalid, 1ULL);
+        if (blockIdx.y == 0) atomicAdd(g.n_invalid, 1ULL);
         return;
     }
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
@@ -160,15 +163,16 @@ k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, con
 }
 
 int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q)
+                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q, int member0, int n_mem)
 {
-    if (n == 0) return PDFB_OK;
-    if (g->d.smem_ok) return pdfb_launch_xfxq2_smem(g, n_req, cols, n, x, q2, out, out_stride, st, q_is_q);
+    if (n == 0 || n_mem == 0) return PDFB_OK;
+    if (g->d.smem_ok) return pdfb_launch_xfxq2_smem(g, n_req, cols, n, x, q2, out, out_stride, st, q_is_q, member0, n_mem);
     ReqCols rc;
     rc.n = n_req;
     for (int r = 0; r < n_req; r++) rc.col[r] = cols[r];
     long long blocks = (n + 255) / 256;
-    k_xfxq2_v0<<<(unsigned)blocks, 256, 0, st>>>(g->d, rc, n, x, q2, out, out_stride, q_is_q);
+    if (n_mem > 65535) return PDFB_ELIMIT;
+    k_xfxq2_v0<<<dim3((unsigned)blocks, (unsigned)n_mem), 256, 0, st>>>(g->d, rc, n, x, q2, out, out_stride, q_is_q, member0);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

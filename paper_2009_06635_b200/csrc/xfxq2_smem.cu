@@ -307,14 +307,16 @@ template <bool Q_IS_Q>  // compile-time: a run-time flag costs 11 % (register pr
 __global__ void __launch_bounds__(NT_SMEM, 1)
 k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
              const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
-             long long out_stride)
+             long long out_stride, int member0, int n_req, int n_jobs)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar;
     __shared__ uint32_t s_wlist[NT_SMEM / 32][32];  // per-warp list of out-of-grid points
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int pass = blockIdx.x % pl.n, seq = blockIdx.x / pl.n, nseq = gridDim.x / pl.n;
-    if (seq >= nseq) return;
+    // job = (member of the set, pass): blockIdx.x = seq * n_jobs + job; a job's CTAs share its tiles
+    const int job = blockIdx.x % n_jobs, seq = blockIdx.x / n_jobs, nseq = gridDim.x / n_jobs;
+    const int pass = job % pl.n, mem = job / pl.n;
+    out += (long long)mem * n_req * out_stride;
     const uint32_t tab = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)g.pre_bytes;
     const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&mbar);
 
@@ -326,7 +328,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     __syncthreads();
     if (tid == 0) {
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(g.slice_bytes) : "memory");
-        const unsigned char *src = reinterpret_cast<const unsigned char *>(g.valg) + (size_t)pl.group[pass] * g.slice_bytes;
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(g.valg) + ((size_t)(member0 + mem) * g.n_groups + pl.group[pass]) * g.slice_bytes;
         for (int o = 0; o < g.slice_bytes; o += 32768) {
             int bytes = min(32768, g.slice_bytes - o);
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -424,7 +426,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
             if (invalid) {
                 store4(out, out_stride, p, row, false, make_double2(qnan, qnan), make_double2(qnan, qnan));
-                if (pass == 0) atomicAdd(g.n_invalid, 1ULL);
+                if (job == 0) atomicAdd(g.n_invalid, 1ULL);
             }
             if (slow_mask) {  // warp-uniform: compact out-of-grid points into this warp's list
                 const int c = __popc(slow_mask);
@@ -461,7 +463,8 @@ int pdfb_smem_eligible(const pdfb_grid *g)
 }
 
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q)
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
+                           int member0, int n_mem)
 {
     // passes: one per (flavour group, distinct use of its columns); duplicates get extra passes
     PassList pl;
@@ -482,14 +485,20 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     }
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
-    int per_pass = sms / pl.n;
-    if (per_pass < 1) per_pass = 1;
+    // jobs = (member, pass).  Few jobs: the SMs are split between them and each CTA is persistent
+    // over its share of the tiles.  More jobs than SMs: one CTA per job over all tiles, scheduled
+    // by the hardware as SMs free up (one CTA per SM at a time: the slice fills shared memory).
+    const long long n_jobs = (long long)pl.n * n_mem;
+    if (n_jobs > 0x3fffffff) return PDFB_ELIMIT;
+    int per_job = (int)(sms / n_jobs);
+    if (per_job < 1) per_job = 1;
     long long tiles = (n + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
-    if (per_pass > tiles) per_pass = (int)tiles;
+    if (per_job > tiles) per_job = (int)tiles;
+    const unsigned grid = (unsigned)(per_job * n_jobs);
     if (q_is_q)
-        k_xfxq2_smem<true><<<per_pass * pl.n, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride);
+        k_xfxq2_smem<true><<<grid, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride, member0, n_req, (int)n_jobs);
     else
-        k_xfxq2_smem<false><<<per_pass * pl.n, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride);
+        k_xfxq2_smem<false><<<grid, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride, member0, n_req, (int)n_jobs);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

@@ -164,6 +164,33 @@ def grid_nnpdf_shaped(sub_scale=None) -> PdfGridSpec:
 
 
 # --------------------------------------------------------------------------
+# PDF sets (SURVEY.md 8(f).1; PAPER.md:171-190, Table 2): N_rep member tables on the knots of
+# the NNPDF-shaped grid, 13 flavours, evaluated on one x-grid of 2415 points at the fitting scale.
+# Stand-in for "N_rep members of NNPDF3.1 NLO" (not available here): member m draws its own
+# family parameters from seed GRID_SEED + 7919 * m.
+# --------------------------------------------------------------------------
+PIDS_13 = (-6, -5, -4, -3, -2, -1, 1, 2, 3, 4, 5, 6, 21)
+FK_POINTS = 2415
+
+
+def grid_member(m: int, pids=PIDS_13) -> PdfGridSpec:
+    return make_pdf_grid(1e-9, 1.0, 100, NNPDF_Q_EDGES, NNPDF_NQ, pids, seed=GRID_SEED + 7919 * int(m))
+
+
+def member_values(n_members: int, pids=PIDS_13, member0: int = 0) -> np.ndarray:
+    """[n_members, table size]: each member's values in LHAPDF grid-file order."""
+    return np.stack([grid_member(member0 + m, pids).values for m in range(n_members)])
+
+
+def queries_fk_xgrid(grid: PdfGridSpec, n: int = FK_POINTS, seed: int = 1006):
+    """x log-uniform over the grid's x range, all at the lowest scale of the grid (Q0 = 1.65 GeV)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    x = np.clip(_log_uniform(rng, float(grid.x_knots[0]), float(grid.x_knots[-1]), n),
+                float(grid.x_knots[0]), float(grid.x_knots[-1]))
+    return x, np.full(n, grid.q2_min, dtype=np.float64)
+
+
+# --------------------------------------------------------------------------
 # alpha_s nodes from one-loop running (closed form; used to FILL the grid and
 # as a pin for the oracle's interpolation, never as the method)
 # --------------------------------------------------------------------------

@@ -510,3 +510,30 @@ def test_scale_bounds_weighted_stencil_sum():
         S = np.abs(wu) @ np.abs(spec.sub_values(s)[:, :, 0]) @ np.abs(wv)
         assert sc >= S * (1 - 1e-12) and sc <= 8 * S + 1e-300
         assert abs(o) <= sc * (1 + 1e-12)
+
+
+# ----------------------------------------------------------------------------------
+# PDF sets: the member helper is the single-member interpolation per table;
+# pinned by what the mathematics fixes -- in range the interpolant is LINEAR in the table values
+# ----------------------------------------------------------------------------------
+def test_member_set_is_linear_in_the_tables():
+    rng = np.random.default_rng(41)
+    xk = rand_knots(rng, 1e-5, 1.0, 9)
+    subs = [rand_knots(rng, 1.5, 4.0, 5), rand_knots(rng, 4.0, 90.0, 6)]
+    pids = [1, 2, 21]
+    size = sum(len(xk) * len(q) * len(pids) for q in subs)
+    f1, f2 = rng.normal(size=size), rng.normal(size=size)
+    a, b = 0.75, -2.5
+    spec = make_spec(xk, subs, pids, values=[np.zeros((len(xk), len(q), len(pids))) for q in subs])
+    x, q2 = W.scan_points(spec, per_cell=4)
+    tabs = np.stack([f1, f2, a * f1 + b * f2])
+    out, sc = oracle.xfxq2_members(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tabs, pids, x, q2,
+                                   with_scale=True)
+    assert out.shape == (3, len(pids), len(x))
+    lin = a * out[0] + b * out[1]
+    S = abs(a) * sc[0] + abs(b) * sc[1]
+    assert np.all(np.abs(out[2] - lin) <= 8e-16 * S + 1e-300), np.max(np.abs(out[2] - lin) / S)
+    # and each member is exactly the single-member oracle on its own table
+    for m in range(3):
+        single = oracle.OraclePdfGrid(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tabs[m]).xfxq2(pids, x, q2)
+        assert np.array_equal(single, out[m])

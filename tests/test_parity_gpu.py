@@ -276,3 +276,58 @@ def test_q_argument_entry_points(torch_cuda, grid2, ograph2, h2):
     assert np.isnan(rc[:3]).all() and np.isfinite(rc[3])
     check_parity(ra, oracle.OracleAlphas.from_spec(aspec).q2(qq), what="alphas_q")
     B.alphas_grid_free(ha)
+
+
+def test_member_set(torch_cuda):
+    """pdf_set_load / pdf_xfxq2_members (Table 2 shape: 13 flavours, 2415 x-points
+    at the fitting scale, N_rep members): every member against the single-member oracle on its own
+    table, member ranges, more jobs than SMs (one CTA per job) and fewer (persistent CTAs), the
+    extrapolation mix, and pdf_xfxq2 = member 0."""
+    torch = torch_cuda
+    n_mem = 60                                   # 60 members x 4 flavour groups = 240 jobs > 148 SMs
+    g0 = W.grid_member(0)
+    vals = W.member_values(n_mem)
+    h = B.pdf_set_load(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals)
+    assert B.pdf_set_members(h) == n_mem and B.pdf_grid_uses_smem_path(h)
+    pids = list(W.PIDS_13)
+    x, q2 = W.queries_fk_xgrid(g0)
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    out = torch.empty((n_mem, len(pids), len(x)), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2_members(h, 0, n_mem, pids, dx, dq, out)
+    torch.cuda.synchronize()
+    ref, sc = oracle.xfxq2_members(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals, pids, x, q2, with_scale=True)
+    check_parity(out.cpu().numpy(), ref, sc, what="member set, FK x-grid")
+    # a member range in the middle, a PID subset, the extrapolation mix (few jobs: persistent CTAs)
+    xm, qm = W.queries_extrapolation_mix(g0, 20_011)
+    sub = [21, -6, 2]
+    dxm, dqm = torch.from_numpy(xm).cuda(), torch.from_numpy(qm).cuda()
+    o2 = torch.empty((3, len(sub), len(xm)), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2_members(h, 7, 3, sub, dxm, dqm, o2)
+    o1 = torch.empty((len(sub), len(xm)), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h, sub, dxm, dqm, o1)
+    torch.cuda.synchronize()
+    r2, s2 = oracle.xfxq2_members(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals[7:10], sub, xm, qm, with_scale=True)
+    check_parity(o2.cpu().numpy(), r2, s2, max_clause_frac=5e-3, what="member range 7..9")
+    r0, s0 = oracle.xfxq2_members(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals[:1], sub, xm, qm, with_scale=True)
+    check_parity(o1.cpu().numpy(), r0[0], s0[0], max_clause_frac=5e-3, what="pdf_xfxq2 = member 0")
+    # argument errors
+    with pytest.raises(B.PdfbError):
+        B.pdf_xfxq2_members(h, n_mem - 1, 2, sub, dxm, dqm, o2)
+    B.pdf_xfxq2_members(h, 0, 0, sub, dxm, dqm, o2)  # empty range: nothing to do
+    B.pdf_grid_free(h)
+    # a set on a tiny grid takes the read-only-cache kernel (member = blockIdx.y)
+    from test_oracle_pins import make_spec, rand_knots
+    rng = np.random.default_rng(5)
+    xk = rand_knots(rng, 1e-4, 1.0, 3)
+    subs = [rand_knots(rng, 1.5, 3.0, 2), rand_knots(rng, 3.0, 9.0, 5)]
+    tv = np.stack([np.concatenate([rng.normal(size=(len(xk), len(q), 2)).reshape(-1) for q in subs]) for _ in range(4)])
+    spec = make_spec(xk, subs, [1, 21], values=[np.zeros((len(xk), len(q), 2)) for q in subs])
+    ht = B.pdf_set_load(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tv)
+    assert not B.pdf_grid_uses_smem_path(ht)
+    xs, qs = W.scan_points(spec, per_cell=4)
+    ot = torch.empty((3, 2, len(xs)), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2_members(ht, 1, 3, [21, 1], torch.from_numpy(xs).cuda(), torch.from_numpy(qs).cuda(), ot)
+    torch.cuda.synchronize()
+    rt, st = oracle.xfxq2_members(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tv[1:4], [21, 1], xs, qs, with_scale=True)
+    check_parity(ot.cpu().numpy(), rt, st, max_clause_frac=1.0, what="tiny member set")
+    B.pdf_grid_free(ht)
