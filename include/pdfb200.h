@@ -38,6 +38,8 @@ enum {
                            share their threshold knot / a subgrid has < 2 Q knots        */
     PDFB_EPID = -3,     /* requested PID not in the grid (PID 0 is an alias of 21)       */
     PDFB_ECUDA = -4,    /* CUDA runtime error (no device, out of memory, launch failure) */
+    PDFB_EIO = -6,      /* a file could not be opened or read                          */
+    PDFB_EFORMAT = -7,  /* a file is not in the expected text layout                   */
     PDFB_ELIMIT = -5    /* more than PDFB_MAX_SUBGRIDS subgrids or PDFB_MAX_PIDS PIDs    */
 };
 #define PDFB_MAX_SUBGRIDS 16
@@ -172,6 +174,31 @@ int pdfb_debug_ln(const double *in, double *out, long long n, void *cuda_stream)
 
 /* Kernels launched by this library since load (all handles); for bench accounting. */
 long long pdfb_launch_count(void);
+
+/*
+ * Host-only front-end for grids in the LHAPDF6 text layout that PDFFlow reads (
+ * SURVEY.md 8(f).2).  Nothing here touches a device: the arrays go to pdf_grid_load /
+ * pdf_set_load / alphas_grid_load.
+ *
+ * Member file ("lhagrid1"): metadata header, then blocks separated by lines "---"; a block is the
+ * x knots (line 1), the Q knots in GeV (line 2), the PIDs (line 3), then nx*nq lines of n_pid
+ * values, x index outer, Q index inner -- pdf_grid_load's own order.  All blocks must share one
+ * x-knot array and one PID list (else PDFB_EKNOTS).  PDFB_EIO: cannot read; PDFB_EFORMAT: not this
+ * layout.  The handle owns host memory until pdfb_lhagrid_free.
+ *   pdfb_lhagrid_get fills caller arrays sized from pdfb_lhagrid_dims:
+ *   x_knots[nx], q_offsets[n_sub+1], q_knots[nq_tot], pids[n_pid], values[nx*nq_tot*n_pid].
+ */
+typedef struct pdfb_lhagrid pdfb_lhagrid;
+int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out);
+int pdfb_lhagrid_dims(const pdfb_lhagrid *g, int *n_sub, int *nx, int *nq_tot, int *n_pid);
+int pdfb_lhagrid_get(const pdfb_lhagrid *g, double *x_knots, int *q_offsets, double *q_knots, int *pids,
+                     double *values);
+void pdfb_lhagrid_free(pdfb_lhagrid *g);
+/* alpha_s nodes of a set's metadata file: the lists AlphaS_Qs (GeV, a repeated Q marks a
+ * threshold) and AlphaS_Vals.  *n = node count; the arrays are filled only if cap >= *n. */
+int pdfb_lhapdf_info_alphas(const char *info_path, int cap, double *q_knots, double *alphas, int *n);
+/* NumMembers of a set's metadata file (1 if the key is absent). */
+int pdfb_lhapdf_info_members(const char *info_path, int *n_members);
 
 /*
  * pdfb_probe -- machine probes for the bounds MEASURED_PEAKS.json does not carry (SURVEY.md 8(d):

@@ -22,7 +22,11 @@ _ll = ctypes.c_longlong
 
 EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
-           "pdfb_launch_count", "pdfb_probe")
+           "pdfb_launch_count", "pdfb_probe", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
+           "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
+
+
+PDFB_EINVAL, PDFB_EKNOTS, PDFB_EPID, PDFB_ECUDA, PDFB_ELIMIT, PDFB_EIO, PDFB_EFORMAT = -1, -2, -3, -4, -5, -6, -7
 
 
 class PdfbError(RuntimeError):
@@ -76,6 +80,18 @@ def lib():
         L.pdfb_strerror.restype = ctypes.c_char_p
         L.pdfb_strerror.argtypes = [ctypes.c_int]
         L.pdfb_launch_count.restype = _ll
+        L.pdfb_lhagrid_read.restype = ctypes.c_int
+        L.pdfb_lhagrid_read.argtypes = [ctypes.c_char_p, ctypes.POINTER(_vp)]
+        L.pdfb_lhagrid_dims.restype = ctypes.c_int
+        L.pdfb_lhagrid_dims.argtypes = [_vp, _ip, _ip, _ip, _ip]
+        L.pdfb_lhagrid_get.restype = ctypes.c_int
+        L.pdfb_lhagrid_get.argtypes = [_vp, _dp, _ip, _dp, _ip, _dp]
+        L.pdfb_lhagrid_free.restype = None
+        L.pdfb_lhagrid_free.argtypes = [_vp]
+        L.pdfb_lhapdf_info_alphas.restype = ctypes.c_int
+        L.pdfb_lhapdf_info_alphas.argtypes = [ctypes.c_char_p, ctypes.c_int, _dp, _dp, _ip]
+        L.pdfb_lhapdf_info_members.restype = ctypes.c_int
+        L.pdfb_lhapdf_info_members.argtypes = [ctypes.c_char_p, _ip]
         L.pdfb_probe.restype = ctypes.c_int
         L.pdfb_probe.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
         L.pdfb_debug_ln.restype = ctypes.c_int
@@ -271,6 +287,62 @@ def alphas_q2_host(a, q2, out):
 
 def alphas_grid_free(a):
     lib().alphas_grid_free(_vp(a))
+
+
+# ------------------------------------------------------------------ LHAPDF text layout (host only)
+def lhagrid_read(path: str):
+    """Parse one member file -> (x_knots, q_offsets, q_knots, pids, values), pdf_grid_load's arguments."""
+    h = _vp()
+    _check(lib().pdfb_lhagrid_read(os.fsencode(path), ctypes.byref(h)), f"pdfb_lhagrid_read({path})")
+    try:
+        d = [ctypes.c_int(0) for _ in range(4)]
+        _check(lib().pdfb_lhagrid_dims(h, *[ctypes.byref(v) for v in d]), "pdfb_lhagrid_dims")
+        n_sub, nx, nq_tot, n_pid = (int(v.value) for v in d)
+        x, q = np.empty(nx), np.empty(nq_tot)
+        off, pids = np.empty(n_sub + 1, np.int32), np.empty(n_pid, np.int32)
+        vals = np.empty(nx * nq_tot * n_pid)
+        _check(lib().pdfb_lhagrid_get(h, x.ctypes.data_as(_dp), off.ctypes.data_as(_ip), q.ctypes.data_as(_dp),
+                                      pids.ctypes.data_as(_ip), vals.ctypes.data_as(_dp)), "pdfb_lhagrid_get")
+    finally:
+        lib().pdfb_lhagrid_free(h)
+    return x, off, q, pids, vals
+
+
+def lhapdf_info_alphas(info_path: str):
+    """-> (q_knots, alphas) of a set's metadata file."""
+    n = ctypes.c_int(0)
+    _check(lib().pdfb_lhapdf_info_alphas(os.fsencode(info_path), 0, None, None, ctypes.byref(n)), "pdfb_lhapdf_info_alphas")
+    q, a = np.empty(n.value), np.empty(n.value)
+    _check(lib().pdfb_lhapdf_info_alphas(os.fsencode(info_path), n.value, q.ctypes.data_as(_dp), a.ctypes.data_as(_dp),
+                                         ctypes.byref(n)), "pdfb_lhapdf_info_alphas")
+    return q, a
+
+
+def lhapdf_info_members(info_path: str) -> int:
+    n = ctypes.c_int(0)
+    _check(lib().pdfb_lhapdf_info_members(os.fsencode(info_path), ctypes.byref(n)), "pdfb_lhapdf_info_members")
+    return int(n.value)
+
+
+def load_lhapdf_set(set_dir: str, members=None, device: int = 0):
+    """Load <set_dir>/<name>_NNNN.dat (name = directory name) as a PDF set and the alpha_s nodes of
+    <name>.info -> (pdf handle, alphas handle).  members: iterable of member numbers (default all)."""
+    name = os.path.basename(os.path.normpath(set_dir))
+    info = os.path.join(set_dir, name + ".info")
+    if members is None:
+        members = range(lhapdf_info_members(info))
+    first, tables = None, []
+    for m in members:
+        x, off, q, pids, vals = lhagrid_read(os.path.join(set_dir, f"{name}_{int(m):04d}.dat"))
+        if first is None:
+            first = (x, off, q, pids)
+        elif not (np.array_equal(x, first[0]) and np.array_equal(off, first[1]) and np.array_equal(q, first[2])
+                  and np.array_equal(pids, first[3])):
+            raise PdfbError(-2, f"member {m} of {name} is on different knots")
+        tables.append(vals)
+    hp = pdf_set_load(first[0], first[1], first[2], first[3], np.stack(tables), device)
+    qa, aa = lhapdf_info_alphas(info)
+    return hp, alphas_grid_load(qa, aa, device)
 
 
 # ------------------------------------------------------------------ spec conveniences

@@ -21,6 +21,8 @@ extern "C" const char *pdfb_strerror(int code)
     case PDFB_EKNOTS: return "bad knots (not increasing, non-positive, sub-grids not sharing their threshold, or < 2 knots)";
     case PDFB_EPID: return "requested PID is not in the grid";
     case PDFB_ECUDA: return "CUDA runtime error (no device, out of memory or launch failure)";
+    case PDFB_EIO: return "file could not be opened or read";
+    case PDFB_EFORMAT: return "file is not in the expected LHAPDF text layout";
     case PDFB_ELIMIT: return "too many sub-grids, PIDs or alpha_s nodes";
     default: return "unknown pdfb error code";
     }

@@ -326,3 +326,30 @@ def scan_points(grid: PdfGridSpec, per_cell: int = 3):
     qs = np.unique(np.clip(np.concatenate(qs), grid.q2_min, grid.q2_max))
     X, Q = np.meshgrid(xs, qs, indexing="ij")
     return np.ascontiguousarray(X.reshape(-1)), np.ascontiguousarray(Q.reshape(-1))
+
+
+# --------------------------------------------------------------------------
+# Writers for the LHAPDF6 text layout (the files themselves are not available here: tests and
+# users write synthetic sets with these and read them back through the library's front-end)
+# --------------------------------------------------------------------------
+def write_lhagrid(spec: PdfGridSpec, path: str, pdf_type: str = "central") -> None:
+    r = lambda a: " ".join(repr(float(v)) for v in a)
+    with open(path, "w") as f:
+        f.write(f"PdfType: {pdf_type}\nFormat: lhagrid1\n---\n")
+        for s in range(spec.n_sub):
+            q = spec.sub_q(s)
+            f.write(r(spec.x_knots) + "\n" + r(q) + "\n" + " ".join(str(int(p)) for p in spec.pids) + "\n")
+            for row in spec.sub_values(s).reshape(spec.nx * len(q), spec.n_pid):
+                f.write(r(row) + "\n")
+            f.write("---\n")
+
+
+def write_lhapdf_info(path: str, n_members: int, pids, alphas_spec) -> None:
+    qs = ", ".join(repr(float(v)) for v in alphas_spec.q_knots)
+    half = len(alphas_spec.alphas) // 2  # a list that continues on a second line, as real files do
+    va = ", ".join(repr(float(v)) for v in alphas_spec.alphas[:half]) + ",\n  " + \
+        ", ".join(repr(float(v)) for v in alphas_spec.alphas[half:])
+    with open(path, "w") as f:
+        f.write(f'SetDesc: "synthetic set written by paper_2009_06635_b200.workloads"\nNumMembers: {int(n_members)}\n')
+        f.write("Flavors: [" + ", ".join(str(int(p)) for p in pids) + "]\nFormat: lhagrid1\n")
+        f.write(f"AlphaS_Type: ipol\nAlphaS_Qs: [{qs}]\nAlphaS_Vals: [{va}]\n")
