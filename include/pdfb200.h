@@ -92,6 +92,9 @@ int pdf_set_members(const pdfb_grid *g);
  */
 int pdf_xfxq2_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
                       long long n, const double *x, const double *q2, double *out, void *cuda_stream);
+/* The same with the scale given as Q in GeV (see pdf_xfxq). */
+int pdf_xfxq_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
+                     long long n, const double *x, const double *q, double *out, void *cuda_stream);
 
 /*
  * pdf_xfxq2 -- xf_pid(x, Q^2) for n points and n_req flavours (section 2.2;

@@ -5,4 +5,6 @@ C-ABI of ``include/pdfb200.h``.  ``binding`` is the thin ctypes layer (argument 
 only); ``workloads`` holds the seeded synthetic input generators.  Importing this package
 does not load the CUDA library; ``binding.lib()`` does and fails loudly if it is missing.
 """
-__all__ = ["binding", "workloads", "build"]
+from .pdf import PDF, mkPDF  # noqa: E402,F401  (the paper's user-facing object; marshalling only)
+
+__all__ = ["binding", "workloads", "build", "PDF", "mkPDF"]

@@ -20,7 +20,7 @@ _ip = ctypes.POINTER(ctypes.c_int)
 _vp = ctypes.c_void_p
 _ll = ctypes.c_longlong
 
-EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
+EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
            "pdfb_launch_count", "pdfb_probe", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
            "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
@@ -53,6 +53,8 @@ def lib():
         L.pdf_set_members.argtypes = [_vp]
         L.pdf_xfxq2_members.restype = ctypes.c_int
         L.pdf_xfxq2_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
+        L.pdf_xfxq_members.restype = ctypes.c_int
+        L.pdf_xfxq_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq2.restype = ctypes.c_int
         L.pdf_xfxq2.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq.restype = ctypes.c_int
@@ -201,11 +203,11 @@ def pdf_set_members(g) -> int:
     return int(lib().pdf_set_members(_vp(g)))
 
 
-def pdf_xfxq2_members(g, member0, n_mem, pids, x, q2, out, stream=None, n=None):
+def pdf_xfxq2_members(g, member0, n_mem, pids, x, q2, out, stream=None, n=None, q_is_q=False):
     """Enqueue members member0..member0+n_mem-1 on the same points -> out[n_mem, n_req, n]."""
     pids = _i32(pids)
     n = int(x.numel() if n is None else n)
-    rc = lib().pdf_xfxq2_members(_vp(g), int(member0), int(n_mem), len(pids), pids.ctypes.data_as(_ip), n,
+    rc = (lib().pdf_xfxq_members if q_is_q else lib().pdf_xfxq2_members)(_vp(g), int(member0), int(n_mem), len(pids), pids.ctypes.data_as(_ip), n,
                                  _dev_ptr(x, n, "x"), _dev_ptr(q2, n, "q2"),
                                  _dev_ptr(out, int(n_mem) * len(pids) * n, "out"), _stream_ptr(stream))
     _check(rc, "pdf_xfxq2_members")
@@ -326,7 +328,7 @@ def lhapdf_info_members(info_path: str) -> int:
 
 def load_lhapdf_set(set_dir: str, members=None, device: int = 0):
     """Load <set_dir>/<name>_NNNN.dat (name = directory name) as a PDF set and the alpha_s nodes of
-    <name>.info -> (pdf handle, alphas handle).  members: iterable of member numbers (default all)."""
+    <name>.info -> (pdf handle, alphas handle, PIDs).  members: iterable of member numbers (default all)."""
     name = os.path.basename(os.path.normpath(set_dir))
     info = os.path.join(set_dir, name + ".info")
     if members is None:
@@ -342,7 +344,7 @@ def load_lhapdf_set(set_dir: str, members=None, device: int = 0):
         tables.append(vals)
     hp = pdf_set_load(first[0], first[1], first[2], first[3], np.stack(tables), device)
     qa, aa = lhapdf_info_alphas(info)
-    return hp, alphas_grid_load(qa, aa, device)
+    return hp, alphas_grid_load(qa, aa, device), first[3]
 
 
 # ------------------------------------------------------------------ spec conveniences

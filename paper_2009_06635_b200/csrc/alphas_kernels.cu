@@ -51,10 +51,15 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
 
 // Fast path (K <= 192 nodes): replicated coefficient lines in shared memory, LUT location,
 // one cubic in t per point.  Two points per thread keep two independent ln chains in flight.
+#ifndef NT_ALPHAS
 #define NT_ALPHAS 512
+#endif
+#ifndef CTAS_ALPHAS
+#define CTAS_ALPHAS 2
+#endif
 
 template <bool Q_IS_Q>
-__global__ void __launch_bounds__(NT_ALPHAS, 2)
+__global__ void __launch_bounds__(NT_ALPHAS, CTAS_ALPHAS)
 k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__restrict__ q2,
               double *__restrict__ out)
 {
@@ -116,7 +121,7 @@ int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, doub
             attr_dev = a->device;
         }
         long long blocks = (n + NT_ALPHAS - 1) / NT_ALPHAS;
-        if (blocks > 148 * 2) blocks = 148 * 2;
+        if (blocks > 148 * CTAS_ALPHAS) blocks = 148 * CTAS_ALPHAS;
         if (q_is_q) k_alphas_fast<true><<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
         else k_alphas_fast<false><<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
         pdfb_count_launch(1);

@@ -249,8 +249,8 @@ extern "C" int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int
 
 extern "C" int pdf_set_members(const pdfb_grid *g) { return g ? g->d.n_members : 0; }
 
-extern "C" int pdf_xfxq2_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
-                                 long long n, const double *x, const double *q2, double *out, void *cuda_stream)
+static int members_impl(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids, long long n,
+                        const double *x, const double *q2, double *out, void *cuda_stream, int q_is_q)
 {
     if (!g || !pids || n < 0 || n_mem < 0) return PDFB_EINVAL;
     if (member0 < 0 || member0 + n_mem > g->d.n_members) return PDFB_EINVAL;
@@ -259,7 +259,19 @@ extern "C" int pdf_xfxq2_members(const pdfb_grid *g, int member0, int n_mem, int
     int rc = resolve_cols(g, n_req, pids, cols);
     if (rc) return rc;
     if (n_mem == 0) return PDFB_OK;
-    return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream, 0, member0, n_mem);
+    return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream, q_is_q, member0, n_mem);
+}
+
+extern "C" int pdf_xfxq2_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
+                                 long long n, const double *x, const double *q2, double *out, void *cuda_stream)
+{
+    return members_impl(g, member0, n_mem, n_req, pids, n, x, q2, out, cuda_stream, 0);
+}
+
+extern "C" int pdf_xfxq_members(const pdfb_grid *g, int member0, int n_mem, int n_req, const int *pids,
+                                long long n, const double *x, const double *q, double *out, void *cuda_stream)
+{
+    return members_impl(g, member0, n_mem, n_req, pids, n, x, q, out, cuda_stream, 1);
 }
 
 extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,

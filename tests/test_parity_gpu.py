@@ -346,8 +346,8 @@ def test_set_loaded_from_lhapdf_layout_files(torch_cuda, tmp_path):
         W.write_lhagrid(sp, str(d / f"synthset_{m:04d}.dat"), "central" if m == 0 else "replica")
     aspec = W.make_alphas_grid()
     W.write_lhapdf_info(str(d / "synthset.info"), 3, pids, aspec)
-    hp, ha = B.load_lhapdf_set(str(d))
-    assert B.pdf_set_members(hp) == 3
+    hp, ha, fpids = B.load_lhapdf_set(str(d))
+    assert B.pdf_set_members(hp) == 3 and list(fpids) == pids
     h_direct = B.pdf_set_load(specs[0].x_knots, specs[0].q_offsets, specs[0].q_knots, specs[0].pids,
                               np.stack([sp.values for sp in specs]))
     x, q2 = W.queries_extrapolation_mix(specs[0], 10_007)
@@ -369,3 +369,35 @@ def test_set_loaded_from_lhapdf_layout_files(torch_cuda, tmp_path):
         B.pdf_grid_free(h)
     for h in (ha, hd):
         B.alphas_grid_free(h)
+
+
+def test_pdf_object_api(torch_cuda, tmp_path):
+    """mkPDF / PDF (Fig. 1): the four interpolating methods and the member form are
+    single calls of the library -- same numbers as the binding calls, from a directory and from specs."""
+    torch = torch_cuda
+    from paper_2009_06635_b200 import PDF, mkPDF
+    d = tmp_path / "objset"
+    d.mkdir()
+    specs = [W.grid_member(m) for m in range(2)]
+    for m, sp in enumerate(specs):
+        W.write_lhagrid(sp, str(d / f"objset_{m:04d}.dat"))
+    aspec = W.make_alphas_grid()
+    W.write_lhapdf_info(str(d / "objset.info"), 2, W.PIDS_13, aspec)
+    x, q2 = W.queries_extrapolation_mix(specs[0], 5_003)
+    q = np.sqrt(q2)
+    with mkPDF(str(d)) as pdf, mkPDF(specs, alphas=aspec) as pdf2:
+        assert isinstance(pdf, PDF) and pdf.n_members == 2 and pdf.pids == tuple(W.PIDS_13)
+        a = pdf.xfxQ2([21, 1], x, q2)
+        b = pdf2.xfxQ2([21, 1], torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda())
+        assert a.shape == (2, len(x)) and torch.equal(a, b)
+        ref, sc = oracle.OraclePdfGrid.from_spec(specs[0]).xfxq2([21, 1], x, q2, with_scale=True)
+        check_parity(a.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what="PDF.xfxQ2")
+        allm = pdf.xfxQ2(None, x, q2, members=(0, 2))
+        assert allm.shape == (2, 13, len(x))
+        assert torch.equal(allm[0, 12], a[0])                         # PID 21 is the last of PIDS_13
+        assert torch.equal(pdf.xfxQ(None, x, q, members=(0, 2)), pdf.xfxQ2(None, x, q * q, members=(0, 2)))
+        assert torch.equal(pdf.xfxQ([2], x, q), pdf.xfxQ2([2], x, q * q))
+        al = pdf.alphasQ2(q2)
+        check_parity(al.cpu().numpy(), oracle.OracleAlphas.from_spec(aspec).q2(q2), what="PDF.alphasQ2")
+        assert torch.equal(pdf.alphasQ(q), pdf.alphasQ2(q * q)) and torch.equal(al, pdf2.alphasQ2(q2))
+        assert pdf.n_invalid() == 0
