@@ -61,6 +61,7 @@ enum {
  *   n_pid,pids host [n_pid], PDG ids of the value columns (e.g. -5..5 and 21)
  *   values     host, xf at the knots, layout [s][ix][iq][ipid] row-major with the sub-grids
  *              concatenated (LHAPDF grid-file order)
+ *              (every value must be finite, else PDFB_EINVAL)
  *   device     CUDA device ordinal
  *   out        receives the handle
  */

@@ -77,6 +77,10 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
         if (s && q_knots[a] != q_knots[a - 1]) return PDFB_EKNOTS;
     }
     const int nq_tot = q_offsets[n_sub];
+    {   // table values must be finite: the kernels multiply out-of-stencil knots by weights that are exactly 0
+        const long long tot = (long long)n_members * nx * nq_tot * n_pid;
+        for (long long e = 0; e < tot; e++) if (!std::isfinite(values[e])) return PDFB_EINVAL;
+    }
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return PDFB_ECUDA;

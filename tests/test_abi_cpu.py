@@ -48,6 +48,13 @@ def test_load_validates_before_cuda(L):
     with pytest.raises(B.PdfbError) as e:  # a sub-grid with one knot
         B.pdf_grid_load(g.x_knots, np.array([0, 1, 15], np.int32), g.q_knots, g.pids, g.values)
     assert e.value.code == -2
+    bad_v = g.values.copy(); bad_v[17] = np.inf       # table values must be finite
+    with pytest.raises(B.PdfbError) as e:
+        B.pdf_grid_load(g.x_knots, g.q_offsets, g.q_knots, g.pids, bad_v)
+    assert e.value.code == -1
+    with pytest.raises(B.PdfbError) as e:             # member count out of range
+        B.pdf_set_load(g.x_knots, g.q_offsets, g.q_knots, g.pids, np.zeros((0, g.values.size)))
+    assert e.value.code == -5
     with pytest.raises(B.PdfbError) as e:
         B.alphas_grid_load([1.0, 2.0, 1.5], [0.3, 0.2, 0.25])
     assert e.value.code == -2
