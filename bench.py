@@ -132,6 +132,54 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def bench_other_configs(torch, B, h, ha, grid, peak):
+    """Configs 1, 2, 4 and 5 of BASELINE.json at their full sizes, device-resident, reported beside
+    the metric (parity-test cases, not the headline): kernel time by CUDA events, 5 repetitions."""
+    def timed(fn, reps=5):
+        for _ in range(2):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record(); torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps
+
+    def dev(*arrs):
+        return [torch.from_numpy(a).cuda() for a in arrs]
+
+    res, p11 = {}, list(W.PIDS_11)
+    g1 = W.grid_config1()
+    h1 = B.load_pdf_spec(g1)
+    x, q2 = dev(*W.queries_in_range(g1, 10_000, 1))
+    o = torch.empty((3, 10_000), dtype=torch.float64, device="cuda")
+    ms = timed(lambda: B.pdf_xfxq2(h1, list(W.PIDS_3), x, q2, o))
+    res["config1_1e4x3"] = {"ms": ms, "evaluations_per_s": 3e4 / (ms * 1e-3), "note": "launch-latency sized"}
+    B.pdf_grid_free(h1)
+    x, q2 = dev(*W.queries_in_range(grid, 1_000_000, 2))
+    o = torch.empty((11, 1_000_000), dtype=torch.float64, device="cuda")
+    ms = timed(lambda: B.pdf_xfxq2(h, p11, x, q2, o))
+    res["config2_1e6x11"] = {"ms": ms, "evaluations_per_s": 1.1e7 / (ms * 1e-3), "hbm_frac": 104e6 / (ms * 1e-3) / 1e9 / peak}
+    n4 = 10_000_000
+    x, q2 = dev(*W.queries_extrapolation_mix(grid, n4))
+    o = torch.empty((11, n4), dtype=torch.float64, device="cuda")
+    ms = timed(lambda: B.pdf_xfxq2(h, p11, x, q2, o))
+    res["config4_mix_1e7x11"] = {"ms": ms, "evaluations_per_s": 11 * n4 / (ms * 1e-3), "hbm_frac": 104 * n4 / (ms * 1e-3) / 1e9 / peak}
+    ms = timed(lambda: B.pdf_xfxq2(h, [21], x, q2, o))
+    res["config4_mix_1e7x1"] = {"ms": ms, "evaluations_per_s": n4 / (ms * 1e-3), "hbm_frac": 24 * n4 / (ms * 1e-3) / 1e9 / peak}
+    x1, x2, q2 = dev(*W.queries_mc_events(grid, n4))
+    o2 = torch.empty((11, n4), dtype=torch.float64, device="cuda")
+    oa = torch.empty(n4, dtype=torch.float64, device="cuda")
+
+    def events():
+        B.pdf_xfxq2(h, p11, x1, q2, o); B.pdf_xfxq2(h, p11, x2, q2, o2); B.alphas_q2(ha, q2, oa)
+    ms = timed(events)
+    res["config5_1e7_events"] = {"ms": ms, "evaluations_per_s": 22 * n4 / (ms * 1e-3), "events_per_s": n4 / (ms * 1e-3),
+                                 "hbm_frac": (2 * 104 + 16) * n4 / (ms * 1e-3) / 1e9 / peak,
+                                 "calls": "pdf_xfxq2(x1), pdf_xfxq2(x2), alphas_q2 on the shared Q^2"}
+    return res
+
+
 def bench_members(torch, B, local, n_rep):
     """SURVEY.md 8(f).1 / PAPER.md:171-190, Table 2: all 13 flavours of N_rep members on a 2415-point
     x-grid, one pdf_xfxq2_members launch; reported beside the metric, not inside it."""
@@ -298,6 +346,8 @@ def run_gpu(args):
                     "unit": "T FP64 op/s (FMA = 1)", "frac": w_f * n / (kern_ms * 1e-3) / fma_ps,
                     "algorithmic_ops_per_point": w_f, "peak_source": "measured: pdfb_probe(PDFB_PROBE_FP64), DFMA chains",
                     "note": "context only; HBM is the slower of the two contract bounds"}
+    if not args.no_other_configs:
+        line["other_configs"] = bench_other_configs(torch, B, h, ha, grid, peak)
     B.alphas_grid_free(ha)
     if not args.no_members:
         line["multi_member"] = bench_members(torch, B, local, args.members)
@@ -321,6 +371,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-members", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--members", type=int, default=400, help="N_rep of the multi-member leg (Table 2)")
     args = ap.parse_args()
     if args.impl == "reference":
