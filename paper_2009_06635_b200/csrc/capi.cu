@@ -142,7 +142,8 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     const int aux_bytes = d.pre_bytes + d.post_bytes;
     size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid * n_members, 128);
     size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_members, 128);
-    size_t total = o_aux + aux_bytes;
+    size_t o_ws = align_up(o_aux + aux_bytes, 128);
+    size_t total = o_ws + PDFB_WS_BYTES;
     char *blob = nullptr;
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
     g->blob = blob; g->blob_bytes = total;
@@ -227,6 +228,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.n_invalid = (unsigned long long *)(blob + o_cnt);
     d.valg = (const double *)(blob + o_valg);
     d.aux = (const unsigned char *)(blob + o_aux);
+    d.slow_ws = (uint32_t *)(blob + o_ws);
     if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
     *out = g;
     return PDFB_OK;

@@ -109,6 +109,7 @@ struct GridDev {
     const IntervalRec *qrec;           // [nq_tot]; entry q_off[s]+j = interval j of sub-grid s
     const double *val;                 // [member][s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
     unsigned long long *n_invalid;     // sticky counter
+    uint32_t *slow_ws;                 // smem path: per-SM, per-warp, per-class lists of out-of-grid points
     // ---- shared-memory path (xfxq2_smem.cu): flavour-group slices + a small aux block
     int smem_ok;                       // 1 if the grid qualifies (nx >= 4, every sub-grid >= 4 Q knots)
     int n_groups, nx4;                 // groups of 4 value columns; nx padded to a multiple of 4
@@ -121,6 +122,9 @@ struct GridDev {
     double lutx_u0, lutx_inv_h, lutq_v0, lutq_inv_h;
 };
 #define PDFB_LUT_BINS 512
+#define PDFB_SLOW_CLASSES 5   // x < x_min | Q^2 > max | Q^2 < min | the two corners
+#define PDFB_WS_SLOTS 256     // >= %nsmid: one scratch slot per SM
+#define PDFB_WS_BYTES (PDFB_WS_SLOTS * 32 * PDFB_SLOW_CLASSES * 32 * 4)  // up to 32 warps per CTA
 // Shared-memory image of the smem path: [pre | slice | post].
 //   pre  = lutx, lutq, raw x knots, raw Q^2 knots, then xrec;   post = qrec, then zero padding.
 // xrec/qrec = 128-byte lines holding 4 copies of the 32-byte IntervalRec32 of an interval (qrec is

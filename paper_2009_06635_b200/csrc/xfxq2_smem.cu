@@ -311,7 +311,6 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar;
-    __shared__ uint32_t s_wlist[NT_SMEM / 32][32];  // per-warp list of out-of-grid points
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     // job = (member of the set, pass): blockIdx.x = seq * n_jobs + job; a job's CTAs share its tiles
     const int job = blockIdx.x % n_jobs, seq = blockIdx.x / n_jobs, nseq = gridDim.x / n_jobs;
@@ -355,14 +354,23 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     const uint32_t RB = sv.row_bytes, rb1 = RB, rb2 = 2u * RB, rb3 = 3u * RB;
     const int row[4] = {pl.row[pass][0], pl.row[pass][1], pl.row[pass][2], pl.row[pass][3]};
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
-    int wcount = 0;  // warp-uniform: entries in this warp's list
-
-    // evaluate the listed out-of-grid points of this warp with (mostly) full lanes
+    // Out-of-grid points are not evaluated where they occur: each warp appends them to one list per
+    // CLASS (0: x < x_min, 1: Q^2 > max, 2: Q^2 < min, 3 and 4: the corners 0+1, 0+2) and evaluates a
+    // list when it holds a warp's worth, so that every slow_point call is class-uniform (no
+    // divergence between the continuation rules) and runs on full lanes.  The lists live in a
+    // global scratch slot owned by this SM (one CTA per SM at a time); counts are warp-uniform,
+    // 6 bits per class in one register.
+    unsigned cnts = 0;
     constexpr int TILE = NT_SMEM * PPT_SMEM;
-    auto flush = [&](int count) {
+    auto wlist = [&]() -> uint32_t * {
+        uint32_t smid;
+        asm("mov.u32 %0, %%smid;" : "=r"(smid));
+        return g.slow_ws + ((size_t)(smid % PDFB_WS_SLOTS) * (NT_SMEM / 32) + warp) * (PDFB_SLOW_CLASSES * 32);
+    };
+    auto flush = [&](int cls, int count) {
         __syncwarp();
         if (lane < count) {
-            const uint32_t e = s_wlist[warp][lane];  // (iteration * PPT + k) << 5 | lane
+            const uint32_t e = __ldcg(wlist() + cls * 32 + lane);  // (iteration * PPT + k) << 5 | lane
             const uint32_t ik = e >> 5;
             const long long ps = ((long long)seq + (long long)(ik / PPT_SMEM) * nseq) * TILE + (ik % PPT_SMEM) * NT_SMEM +
                                  warp * 32 + (e & 31);
@@ -428,20 +436,33 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                 store4(out, out_stride, p, row, false, make_double2(qnan, qnan), make_double2(qnan, qnan));
                 if (job == 0) atomicAdd(g.n_invalid, 1ULL);
             }
-            if (slow_mask) {  // warp-uniform: compact out-of-grid points into this warp's list
-                const int c = __popc(slow_mask);
-                if (wcount + c > 32) { flush(wcount); wcount = 0; }
-                if (slow) s_wlist[warp][wcount + __popc(slow_mask & ((1u << lane) - 1u))] = ((it * PPT_SMEM + k) << 5) | (uint32_t)lane;
-                wcount += c;
+            if (slow_mask) {  // warp-uniform: append the out-of-grid points to their class lists
+                const bool low_x = xv[k] < g.x_min, high_q = qv[k] > g.q2_max, low_q = qv[k] < g.q2_min;
+                const int cls = low_x ? (high_q ? 3 : (low_q ? 4 : 0)) : (high_q ? 1 : 2);
+                uint32_t *wl = wlist();
+#pragma unroll
+                for (int c = 0; c < PDFB_SLOW_CLASSES; c++) {
+                    const unsigned m = __ballot_sync(0xffffffffu, slow && cls == c);
+                    if (m) {
+                        const int kc = __popc(m);
+                        int cur = (cnts >> (6 * c)) & 63;
+                        if (cur + kc > 32) { flush(c, cur); cur = 0; }
+                        if (slow && cls == c)
+                            __stcg(wl + c * 32 + cur + __popc(m & ((1u << lane) - 1u)), ((it * PPT_SMEM + k) << 5) | (uint32_t)lane);
+                        cnts = (cnts & ~(63u << (6 * c))) | ((unsigned)(cur + kc) << (6 * c));
+                    }
+                }
             }
             xv[k] = xn[k]; qv[k] = qn[k];
         }
     }
-    if (wcount) flush(wcount);
+#pragma unroll
+    for (int c = 0; c < PDFB_SLOW_CLASSES; c++)
+        if ((cnts >> (6 * c)) & 63) flush(c, (cnts >> (6 * c)) & 63);
 }
 
 static int smem_needed(const GridDev &d) { return d.pre_bytes + d.slice_bytes + d.post_bytes; }
-static const int STATIC_SMEM = 64 + NT_SMEM * 4 + 256;  // >= the kernel's static shared memory (mbarrier, list)
+static const int STATIC_SMEM = 256;  // >= the kernel's static shared memory (mbarrier)
 
 int pdfb_smem_eligible(const pdfb_grid *g)
 {
