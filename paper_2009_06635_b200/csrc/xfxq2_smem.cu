@@ -47,13 +47,25 @@ __device__ __forceinline__ double2 lds128(uint32_t addr)
     return v;
 }
 
-__device__ __forceinline__ double cont_e(double r, double yL, double yH)  // reading O4
+// The continuation rules run on a few percent of the points at most but carry the fp64 log / exp /
+// pow bodies: they are kept OUT of line (one copy each) so that the kernel stays within the
+// instruction cache when warps alternate between the fast path and the out-of-grid lists
+// (inlined they made the kernel 112 KB and a 30 % out-of-grid mix 3x slower than its parts).
+__device__ __noinline__ double cont_e(double r, double yL, double yH)  // reading O4
 {
     if (yL > 1e-3 && yH > 1e-3) {
         double lL = log(yL);
         return exp(fma(r, log(yH) - lL, lL));
     }
     return fma(r, yH - yL, yL);
+}
+
+// rule C (reading O5): y0 * rho^(gamma*rho + 1 - rho), gamma from the probe at 1.01 q_min
+__device__ __noinline__ double rule_c(double y0, double y1, double rho)
+{
+    double gamma = 0.0;
+    if (fabs(y0) >= 1e-5) gamma = fmax(-2.5, (y1 - y0) / y0 / 0.01);
+    return y0 * pow(rho, fma(gamma, rho, 1.0 - rho));
 }
 
 // The four 1-D weights of knots m-1..m+2 from the 32-byte interval record.  aLm == 0 marks the
@@ -197,6 +209,17 @@ __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, d
 
 struct Y4 { double2 E, O; };  // column pair (lane & 1) and the other pair
 
+// one stencil evaluation of the out-of-grid path, out of line (see cont_e)
+__device__ __noinline__ Y4 probe4(uint32_t row0, uint32_t RB, int node0, const double *wu, const double *vw, int lane8)
+{
+    const double wu4[4] = {wu[0], wu[1], wu[2], wu[3]}, vw4[4] = {vw[0], vw[1], vw[2], vw[3]};
+    Win w;
+    make_win(w, row0, node0, wu4, lane8);
+    Y4 r;
+    gather4(w, vw4, RB, 2 * RB, 3 * RB, r.E, r.O);
+    return r;
+}
+
 // points outside the grid (readings O4/O5): up to 2 x-sets times 2 row sets
 __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
 {
@@ -241,26 +264,21 @@ __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, do
     }
     const bool two_v = high_q || low_q;
     double y1[4], y2[4] = {0.0, 0.0, 0.0, 0.0};
-    double2 E, O;
-    Win w;
-    make_win(w, sv.tab + (uint32_t)(row1 * (int)RB), node0, wu1, lane8);
-    gather4(w, vw1, RB, 2 * RB, 3 * RB, E, O);
-    y1[0] = E.x; y1[1] = E.y; y1[2] = O.x; y1[3] = O.y;
+    const uint32_t r1 = sv.tab + (uint32_t)(row1 * (int)RB), r2 = sv.tab + (uint32_t)(row2 * (int)RB);
+    Y4 p = probe4(r1, RB, node0, wu1, vw1, lane8);
+    y1[0] = p.E.x; y1[1] = p.E.y; y1[2] = p.O.x; y1[3] = p.O.y;
     if (two_v) {
-        make_win(w, sv.tab + (uint32_t)(row2 * (int)RB), node0, wu1, lane8);
-        gather4(w, vw2, RB, 2 * RB, 3 * RB, E, O);
-        y2[0] = E.x; y2[1] = E.y; y2[2] = O.x; y2[3] = O.y;
+        p = probe4(r2, RB, node0, wu1, vw2, lane8);
+        y2[0] = p.E.x; y2[1] = p.E.y; y2[2] = p.O.x; y2[3] = p.O.y;
     }
     if (low_x) {
-        make_win(w, sv.tab + (uint32_t)(row1 * (int)RB), 0, wu2, lane8);
-        gather4(w, vw1, RB, 2 * RB, 3 * RB, E, O);
-        const double h1[4] = {E.x, E.y, O.x, O.y};
+        p = probe4(r1, RB, 0, wu2, vw1, lane8);
+        const double h1[4] = {p.E.x, p.E.y, p.O.x, p.O.y};
 #pragma unroll
         for (int k = 0; k < 4; k++) y1[k] = cont_e(rA, y1[k], h1[k]);
         if (two_v) {
-            make_win(w, sv.tab + (uint32_t)(row2 * (int)RB), 0, wu2, lane8);
-            gather4(w, vw2, RB, 2 * RB, 3 * RB, E, O);
-            const double h2[4] = {E.x, E.y, O.x, O.y};
+            p = probe4(r2, RB, 0, wu2, vw2, lane8);
+            const double h2[4] = {p.E.x, p.E.y, p.O.x, p.O.y};
 #pragma unroll
             for (int k = 0; k < 4; k++) y2[k] = cont_e(rA, y2[k], h2[k]);
         }
@@ -268,15 +286,8 @@ __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, do
     const double rho = qv / g.q2_min;
 #pragma unroll
     for (int k = 0; k < 4; k++) {
-        double r = y1[k];
-        if (high_q) {
-            r = cont_e(rB, y1[k], y2[k]);
-        } else if (low_q) {
-            double gamma = 0.0;
-            if (fabs(y1[k]) >= 1e-5) gamma = fmax(-2.5, (y2[k] - y1[k]) / y1[k] / 0.01);
-            r = y1[k] * pow(rho, fma(gamma, rho, 1.0 - rho));
-        }
-        y1[k] = r;
+        if (high_q) y1[k] = cont_e(rB, y1[k], y2[k]);
+        else if (low_q) y1[k] = rule_c(y1[k], y2[k], rho);
     }
     Y4 res;
     res.E = make_double2(y1[0], y1[1]);
