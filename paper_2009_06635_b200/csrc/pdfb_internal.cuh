@@ -121,7 +121,9 @@ struct GridDev {
     int a_qrec;                        // byte offset inside post (its head)
     double lutx_u0, lutx_inv_h, lutq_v0, lutq_inv_h;
 };
+#ifndef PDFB_LUT_BINS
 #define PDFB_LUT_BINS 512
+#endif
 #define PDFB_SLOW_CLASSES 5   // x < x_min | Q^2 > max | Q^2 < min | the two corners
 #define PDFB_WS_SLOTS 256     // >= %nsmid: one scratch slot per SM
 #define PDFB_WS_BYTES (PDFB_WS_SLOTS * 32 * PDFB_SLOW_CLASSES * 32 * 4)  // up to 32 warps per CTA
