@@ -135,9 +135,9 @@ int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points);
 double pdf_grid_setup_ms(const pdfb_grid *g);
 
 /* 1 if pdf_xfxq2 on this handle runs the shared-memory kernel (grid qualifies: nx >= 4, every
- * sub-grid >= 4 Q knots, one 4-column slice fits shared memory), 0 if it runs the
- * read-only-cache fallback kernel.  Setting PDFB_FORCE_FALLBACK in the environment before
- * pdf_grid_load forces 0 (testing). */
+ * sub-grid >= 4 Q knots, a 4-column or at least a 2-column slice of the table fits shared memory),
+ * 0 if it runs the read-only-cache fallback kernel.  Setting PDFB_FORCE_FALLBACK in the
+ * environment before pdf_grid_load forces 0, PDFB_NO_W4 forces the 2-column slices (testing). */
 int pdf_grid_uses_smem_path(const pdfb_grid *g);
 
 void pdf_grid_free(pdfb_grid *g);

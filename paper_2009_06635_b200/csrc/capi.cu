@@ -126,6 +126,9 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.nx4 = (nx + 3) & ~3;
     d.n_groups = (n_pid + 3) / 4;
     d.slice_bytes = nq_tot * d.nx4 * 32;
+    d.nx2 = nx + ((4 - nx % 8) + 8) % 8;  // smallest >= nx that is 4 (mod 8)
+    d.n_groups2 = (n_pid + 1) / 2;
+    d.slice2_bytes = nq_tot * d.nx2 * 16;
     d.smem_ok = (nx >= 4);
     for (int s = 0; s < n_sub; s++) if (q_offsets[s + 1] - q_offsets[s] < 4) d.smem_ok = 0;
     if (nq_tot >= 8192 || nx >= 8192) d.smem_ok = 0;  // LUT entry bit budget
@@ -141,7 +144,8 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     if (128 * nx < d.nx4 * 32 + 32) d.smem_ok = 0;  // (never: 128 nx >= 32 nx4 + 32 for nx >= 2)
     const int aux_bytes = d.pre_bytes + d.post_bytes;
     size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid * n_members, 128);
-    size_t o_aux = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_members, 128);
+    size_t o_valg2 = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_members, 128);
+    size_t o_aux = align_up(o_valg2 + (size_t)d.slice2_bytes * d.n_groups2 * n_members, 128);
     size_t o_ws = align_up(o_aux + aux_bytes, 128);
     size_t total = o_ws + PDFB_WS_BYTES;
     char *blob = nullptr;
@@ -197,6 +201,10 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
                 if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src, valg_m,
                                                       q_offsets[s] * d.nx4, nx, d.nx4, nq, n_pid, d.n_groups,
                                                       (long long)d.slice_bytes / 8, 0);
+                if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src,
+                                                      (double *)(blob + o_valg2) + (long long)m * d.n_groups2 * (d.slice2_bytes / 8),
+                                                      q_offsets[s] * d.nx2, nx, d.nx2, nq, n_pid, d.n_groups2,
+                                                      (long long)d.slice2_bytes / 8, 0, 2);
                 src += (long long)nx * nq * n_pid;
             }
         }
@@ -227,6 +235,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.val = (const double *)(blob + o_val);
     d.n_invalid = (unsigned long long *)(blob + o_cnt);
     d.valg = (const double *)(blob + o_valg);
+    d.valg2 = (const double *)(blob + o_valg2);
     d.aux = (const unsigned char *)(blob + o_aux);
     d.slow_ws = (uint32_t *)(blob + o_ws);
     if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
@@ -302,7 +311,7 @@ extern "C" int pdf_xfxq(const pdfb_grid *g, int n_req, const int *pids, long lon
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q, out, n, (cudaStream_t)cuda_stream, 1);
 }
 
-extern "C" int pdf_grid_uses_smem_path(const pdfb_grid *g) { return g ? g->d.smem_ok : 0; }
+extern "C" int pdf_grid_uses_smem_path(const pdfb_grid *g) { return g ? (g->d.smem_ok != 0) : 0; }
 
 extern "C" int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points)
 {

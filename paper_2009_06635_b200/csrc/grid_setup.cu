@@ -67,22 +67,23 @@ __global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *_
     }
 }
 
-// values of one sub-grid: file order [ix][iq][ipid] -> flavour-group slices [g][iq][ix4][4]
-// (the shared-memory path stages one slice per CTA); padding columns / knots = 0
+// values of one sub-grid: file order [ix][iq][ipid] -> flavour-group slices [g][iq][nxp][W]
+// (the shared-memory path stages one slice per CTA; W = 4 or 2 columns per group, nxp = padded
+// knots per row); padding columns / knots = 0
 __global__ void k1_group_slices(const double *__restrict__ src, double *__restrict__ valg, int s_knot_off,
-                                int nx, int nx4, int nq, int n_pid, int n_groups, long long group_stride)
+                                int nx, int nxp, int nq, int n_pid, int n_groups, long long group_stride, int W)
 {
-    long long tot = (long long)n_groups * nq * nx4 * 4;
+    long long tot = (long long)n_groups * nq * nxp * W;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
          e += (long long)gridDim.x * blockDim.x) {
-        int slot = (int)(e & 3);
-        long long r = e >> 2;
-        int ix = (int)(r % nx4); r /= nx4;
+        int slot = (int)(e % W);
+        long long r = e / W;
+        int ix = (int)(r % nxp); r /= nxp;
         int iq = (int)(r % nq);
         int grp = (int)(r / nq);
-        int k = grp * 4 + slot;
+        int k = grp * W + slot;
         double v = (ix < nx && k < n_pid) ? src[((long long)ix * nq + iq) * n_pid + k] : 0.0;
-        valg[grp * group_stride + ((long long)(s_knot_off + iq * nx4 + ix)) * 4 + slot] = v;
+        valg[grp * group_stride + ((long long)(s_knot_off + iq * nxp + ix)) * W + slot] = v;
     }
 }
 
@@ -126,12 +127,12 @@ int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_
 }
 
 int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
-                            int n_pid, int n_groups, long long group_stride, cudaStream_t st)
+                            int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W)
 {
-    long long tot = (long long)n_groups * nq * nx4 * 4;
+    long long tot = (long long)n_groups * nq * nx4 * W;
     int blocks = (int)((tot + 255) / 256);
     if (blocks > 1184) blocks = 1184;
-    k1_group_slices<<<blocks, 256, 0, st>>>(d_src, d_valg, s_knot_off, nx, nx4, nq, n_pid, n_groups, group_stride);
+    k1_group_slices<<<blocks, 256, 0, st>>>(d_src, d_valg, s_knot_off, nx, nx4, nq, n_pid, n_groups, group_stride, W);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

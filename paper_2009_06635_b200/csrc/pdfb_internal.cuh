@@ -111,10 +111,16 @@ struct GridDev {
     unsigned long long *n_invalid;     // sticky counter
     uint32_t *slow_ws;                 // smem path: per-SM, per-warp, per-class lists of out-of-grid points
     // ---- shared-memory path (xfxq2_smem.cu): flavour-group slices + a small aux block
-    int smem_ok;                       // 1 if the grid qualifies (nx >= 4, every sub-grid >= 4 Q knots)
+    int smem_ok;                       // bit 0: the 4-column slices fit shared memory; bit 1: the 2-column ones
+                                       // (0 if nx < 4 or a sub-grid has < 4 Q knots: read-only-cache kernel)
     int n_groups, nx4;                 // groups of 4 value columns; nx padded to a multiple of 4
     int slice_bytes;                   // one group's slice: nq_tot * nx4 * 32 B
     const double *valg;                // [member][group][s][iq][ix4][4]
+    // 2-column slices: half the bytes per knot, for grids whose 4-column slice exceeds shared memory
+    // and for requests of one or two flavours.  nx2 = 4 (mod 8), so that a row is 64 (mod 128) bytes
+    // long and two consecutive rows of a 4-knot run cover all 8 bank groups (xfxq2_smem.cu)
+    int n_groups2, nx2, slice2_bytes;
+    const double *valg2;               // [member][group2][s][iq][nx2][2]
     const unsigned char *aux;          // [pre | post] blocks, copied verbatim around the slice
     int pre_bytes, post_bytes;         // shared memory = [pre | slice | post]
     int a_xk, a_q2k, a_lutx, a_lutq, a_xrec;  // byte offsets inside pre (a_xrec is its tail)
@@ -200,7 +206,7 @@ int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, doub
 int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_rec32, int n_arrays,
                        const int *h_off, cudaStream_t st);
 int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
-                            int n_pid, int n_groups, long long group_stride, cudaStream_t st);
+                            int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W = 4);
 int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
                            const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,

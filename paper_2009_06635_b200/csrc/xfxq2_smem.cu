@@ -142,21 +142,77 @@ __device__ __forceinline__ void gather4(const Win &u, const double vw[4], uint32
     }
 }
 
+// ---- 2-column slices (16 B per knot).  A 4-knot run is 64 bytes = 4 bank groups; the row length is
+// 64 (mod 128) bytes, so the same run one row further down covers the other 4.  A ROW PAIR is read as
+// one virtual run of 8 chunks: chunk v < 4 = (upper row, knot v), v >= 4 = (lower row, knot v - 4),
+// bank group (g0 + v) & 7.  Lane l reads v(s) = (s + l - g0) & 7 at step s: the 8 lanes of a
+// quarter-warp are on 8 distinct bank groups whatever their cells.  16 conflict-free LDS.128 per
+// point, each delivering both columns of one knot (no column-pair parity here).
+__device__ __forceinline__ void stencil2(uint32_t row0, uint32_t RB, int node0, const double wu[4], const double vw[4],
+                                         int lane8, double out[2])
+{
+    const uint32_t base = row0 + (uint32_t)(node0 * 16);
+    const int rho = (lane8 - (int)(base >> 4)) & 7;  // g0 = bank group of the run's first chunk
+    double Wr[4];
+    rot4(wu, rho & 3, Wr);  // Wr[j] = weight of the knot read at steps s = j, j + 4
+    uint32_t a[8];
+    bool low[8];            // step s reads the lower row of the pair
+#pragma unroll
+    for (int s = 0; s < 8; s++) {
+        const int v = (s + rho) & 7;
+        low[s] = v >> 2;
+        a[s] = base + (uint32_t)((v & 3) << 4) + (low[s] ? RB : 0u);
+    }
+    double y0 = 0.0, y1 = 0.0;
+#pragma unroll
+    for (int p = 0; p < 2; p++) {  // row pairs (0,1) and (2,3)
+        double2 c[8];
+#pragma unroll
+        for (int s = 0; s < 8; s++) c[s] = lds128(a[s] + (p ? 2u * RB : 0u));
+#pragma unroll
+        for (int s = 0; s < 8; s++) {
+            const double w = Wr[s & 3] * (low[s] ? vw[2 * p + 1] : vw[2 * p]);
+            y0 = fma(w, c[s].x, y0); y1 = fma(w, c[s].y, y1);
+        }
+    }
+    out[0] = y0; out[1] = y1;
+}
+
+// One stencil evaluation on a W-column slice: first stencil row `row` (table row gi-1), first knot
+// node0 (= i-1); values come back in column order.
+template <int W>
+__device__ __forceinline__ void eval_stencil(uint32_t tab, uint32_t RB, uint32_t RB2, uint32_t RB3, int row, int node0,
+                                             const double wu[4], const double vw[4], int lane8, double out[W])
+{
+    const uint32_t row0 = tab + (uint32_t)(row * (int)RB);
+    if (W == 4) {
+        Win w;
+        make_win(w, row0, node0, wu, lane8);
+        double2 E, O;
+        gather4(w, vw, RB, RB2, RB3, E, O);
+        const bool odd = lane8 & 1;  // E / O are the column pairs (lane & 1) / the other: back to column order
+        out[0] = odd ? O.x : E.x; out[1] = odd ? O.y : E.y; out[W - 2] = odd ? E.x : O.x; out[W - 1] = odd ? E.y : O.y;
+    } else {
+        stencil2(row0, RB, node0, wu, vw, lane8, out);
+    }
+}
+
 struct SmemViews {
     uint32_t tab, row_bytes, xrec, qrec;  // shared-space byte addresses
     const double *xk, *q2k;
     const unsigned short *lutx, *lutq;
 };
 
-// shared memory = [pre | slice | post] (pdfb_internal.cuh)
+// shared memory = [pre | slice | post] (pdfb_internal.cuh); the slice has W columns per knot
+template <int W>
 __device__ __forceinline__ SmemViews make_views(const GridDev &g, unsigned char *smem)
 {
     SmemViews sv;
     const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(smem);
     sv.tab = s0 + (uint32_t)g.pre_bytes;
-    sv.row_bytes = (uint32_t)g.nx4 * 32u;
+    sv.row_bytes = (W == 4) ? (uint32_t)g.nx4 * 32u : (uint32_t)g.nx2 * 16u;
     sv.xrec = s0 + (uint32_t)g.a_xrec;
-    sv.qrec = sv.tab + (uint32_t)(g.slice_bytes + g.a_qrec);
+    sv.qrec = sv.tab + (uint32_t)((W == 4 ? g.slice_bytes : g.slice2_bytes) + g.a_qrec);
     sv.xk = reinterpret_cast<const double *>(smem + g.a_xk);
     sv.q2k = reinterpret_cast<const double *>(smem + g.a_q2k);
     sv.lutx = reinterpret_cast<const unsigned short *>(smem + g.a_lutx);
@@ -207,24 +263,24 @@ __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, d
     return min(locate(sv.lutq, sv.q2k, g.nq_tot - 1, qv, v, g.lutq_v0, g.lutq_inv_h), g.nq_tot - 2);
 }
 
-struct Y4 { double2 E, O; };  // column pair (lane & 1) and the other pair
+template <int W> struct YW { double v[W]; };  // one point's W columns, in column order
 
 // one stencil evaluation of the out-of-grid path, out of line (see cont_e)
-__device__ __noinline__ Y4 probe4(uint32_t row0, uint32_t RB, int node0, const double *wu, const double *vw, int lane8)
+template <int W>
+__device__ __noinline__ YW<W> probe(uint32_t tab, uint32_t RB, int row, int node0, const double *wu, const double *vw, int lane8)
 {
     const double wu4[4] = {wu[0], wu[1], wu[2], wu[3]}, vw4[4] = {vw[0], vw[1], vw[2], vw[3]};
-    Win w;
-    make_win(w, row0, node0, wu4, lane8);
-    Y4 r;
-    gather4(w, vw4, RB, 2 * RB, 3 * RB, r.E, r.O);
+    YW<W> r;
+    eval_stencil<W>(tab, RB, 2u * RB, 3u * RB, row, node0, wu4, vw4, lane8, r.v);
     return r;
 }
 
 // points outside the grid (readings O4/O5): up to 2 x-sets times 2 row sets
-__device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
+template <int W>
+__device__ __noinline__ YW<W> slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
 {
     const GridDev &g = *gp;
-    const SmemViews sv = make_views(g, smem);
+    const SmemViews sv = make_views<W>(g, smem);
     const uint32_t RB = sv.row_bytes;
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
     // ---- x: one weight set in range, else the two one-hot sets of knots 0 and 1 (rule A)
@@ -263,47 +319,38 @@ __device__ __noinline__ Y4 slow_point(const GridDev *gp, unsigned char *smem, do
         row1 = row2 = gi - 1;
     }
     const bool two_v = high_q || low_q;
-    double y1[4], y2[4] = {0.0, 0.0, 0.0, 0.0};
-    const uint32_t r1 = sv.tab + (uint32_t)(row1 * (int)RB), r2 = sv.tab + (uint32_t)(row2 * (int)RB);
-    Y4 p = probe4(r1, RB, node0, wu1, vw1, lane8);
-    y1[0] = p.E.x; y1[1] = p.E.y; y1[2] = p.O.x; y1[3] = p.O.y;
-    if (two_v) {
-        p = probe4(r2, RB, node0, wu1, vw2, lane8);
-        y2[0] = p.E.x; y2[1] = p.E.y; y2[2] = p.O.x; y2[3] = p.O.y;
-    }
+    YW<W> y1 = probe<W>(sv.tab, RB, row1, node0, wu1, vw1, lane8), y2 = y1;
+    if (two_v) y2 = probe<W>(sv.tab, RB, row2, node0, wu1, vw2, lane8);
     if (low_x) {
-        p = probe4(r1, RB, 0, wu2, vw1, lane8);
-        const double h1[4] = {p.E.x, p.E.y, p.O.x, p.O.y};
+        const YW<W> h1 = probe<W>(sv.tab, RB, row1, 0, wu2, vw1, lane8);
 #pragma unroll
-        for (int k = 0; k < 4; k++) y1[k] = cont_e(rA, y1[k], h1[k]);
+        for (int k = 0; k < W; k++) y1.v[k] = cont_e(rA, y1.v[k], h1.v[k]);
         if (two_v) {
-            p = probe4(r2, RB, 0, wu2, vw2, lane8);
-            const double h2[4] = {p.E.x, p.E.y, p.O.x, p.O.y};
+            const YW<W> h2 = probe<W>(sv.tab, RB, row2, 0, wu2, vw2, lane8);
 #pragma unroll
-            for (int k = 0; k < 4; k++) y2[k] = cont_e(rA, y2[k], h2[k]);
+            for (int k = 0; k < W; k++) y2.v[k] = cont_e(rA, y2.v[k], h2.v[k]);
         }
     }
     const double rho = qv / g.q2_min;
 #pragma unroll
-    for (int k = 0; k < 4; k++) {
-        if (high_q) y1[k] = cont_e(rB, y1[k], y2[k]);
-        else if (low_q) y1[k] = rule_c(y1[k], y2[k], rho);
+    for (int k = 0; k < W; k++) {
+        if (high_q) y1.v[k] = cont_e(rB, y1.v[k], y2.v[k]);
+        else if (low_q) y1.v[k] = rule_c(y1.v[k], y2.v[k], rho);
     }
-    Y4 res;
-    res.E = make_double2(y1[0], y1[1]);
-    res.O = make_double2(y1[2], y1[3]);
-    return res;
+    return y1;
 }
 
-// E / O are the column pairs (lane & 1) / the other: put them back in column order and store
-__device__ __forceinline__ void store4(double *__restrict__ out, long long out_stride, long long p,
-                                       const int row[4], bool odd, double2 E, double2 O)
+// one point's W columns to their output rows (row < 0: column not requested)
+template <int W>
+__device__ __forceinline__ void store_cols(double *__restrict__ out, long long out_stride, long long p,
+                                           const int row[W], const double v[W])
 {
-    const double c0 = odd ? O.x : E.x, c1 = odd ? O.y : E.y, c2 = odd ? E.x : O.x, c3 = odd ? E.y : O.y;
-    if (row[0] >= 0) __stcs(out + row[0] * out_stride + p, c0);
-    if (row[1] >= 0) __stcs(out + row[1] * out_stride + p, c1);
-    if (row[2] >= 0) __stcs(out + row[2] * out_stride + p, c2);
-    if (row[3] >= 0) __stcs(out + row[3] * out_stride + p, c3);
+    if (row[0] >= 0) __stcs(out + row[0] * out_stride + p, v[0]);
+    if (row[1] >= 0) __stcs(out + row[1] * out_stride + p, v[1]);
+    if (W == 4) {
+        if (row[W - 2] >= 0) __stcs(out + row[W - 2] * out_stride + p, v[W - 2]);
+        if (row[W - 1] >= 0) __stcs(out + row[W - 1] * out_stride + p, v[W - 1]);
+    }
 }
 
 // the scale of a point: Q^2, or Q in GeV squared once on load (a non-positive Q is invalid, like Q^2 <= 0)
@@ -314,7 +361,7 @@ __device__ __forceinline__ double load_scale(const double *p)
     return Q_IS_Q ? ((q > 0.0) ? q * q : -1.0) : q;
 }
 
-template <bool Q_IS_Q>  // compile-time: a run-time flag costs 11 % (register pressure at the 128 cap)
+template <bool Q_IS_Q, int W>  // compile-time: a run-time flag costs 11 % (register pressure at the 128 cap)
 __global__ void __launch_bounds__(NT_SMEM, 1)
 k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
              const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
@@ -329,6 +376,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     out += (long long)mem * n_req * out_stride;
     const uint32_t tab = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)g.pre_bytes;
     const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&mbar);
+    const int slice_bytes = (W == 4) ? g.slice_bytes : g.slice2_bytes;
 
     // ---- stage this CTA's flavour-group slice with TMA bulk copies; small tables by plain loads
     if (tid == 0) {
@@ -337,17 +385,18 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     }
     __syncthreads();
     if (tid == 0) {
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(g.slice_bytes) : "memory");
-        const unsigned char *src = reinterpret_cast<const unsigned char *>(g.valg) + ((size_t)(member0 + mem) * g.n_groups + pl.group[pass]) * g.slice_bytes;
-        for (int o = 0; o < g.slice_bytes; o += 32768) {
-            int bytes = min(32768, g.slice_bytes - o);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(slice_bytes) : "memory");
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(W == 4 ? g.valg : g.valg2) +
+                                   ((size_t)(member0 + mem) * (W == 4 ? g.n_groups : g.n_groups2) + pl.group[pass]) * slice_bytes;
+        for (int o = 0; o < slice_bytes; o += 32768) {
+            int bytes = min(32768, slice_bytes - o);
             asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                          ::"r"(tab + o), "l"(src + o), "r"(bytes), "r"(mb) : "memory");
         }
     }
     {   // pre and post blocks around the slice (both multiples of 128 bytes)
         const int4 *src = reinterpret_cast<const int4 *>(g.aux);
-        int4 *pre = reinterpret_cast<int4 *>(smem), *post = reinterpret_cast<int4 *>(smem + g.pre_bytes + g.slice_bytes);
+        int4 *pre = reinterpret_cast<int4 *>(smem), *post = reinterpret_cast<int4 *>(smem + g.pre_bytes + slice_bytes);
         const int npre = g.pre_bytes / 16, npost = g.post_bytes / 16;
         for (int e = tid; e < npre; e += NT_SMEM) pre[e] = __ldg(src + e);
         for (int e = tid; e < npost; e += NT_SMEM) post[e] = __ldg(src + npre + e);
@@ -359,10 +408,10 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
                          : "=r"(done) : "r"(mb) : "memory");
     }
-    const SmemViews sv = make_views(g, smem);
+    const SmemViews sv = make_views<W>(g, smem);
     const int lane8 = tid & 7;
+    const uint32_t RB = sv.row_bytes, rb2 = 2u * RB, rb3 = 3u * RB;
     const bool odd = lane8 & 1;
-    const uint32_t RB = sv.row_bytes, rb1 = RB, rb2 = 2u * RB, rb3 = 3u * RB;
     const int row[4] = {pl.row[pass][0], pl.row[pass][1], pl.row[pass][2], pl.row[pass][3]};
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
     // Out-of-grid points are not evaluated where they occur: each warp appends them to one list per
@@ -385,8 +434,8 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const uint32_t ik = e >> 5;
             const long long ps = ((long long)seq + (long long)(ik / PPT_SMEM) * nseq) * TILE + (ik % PPT_SMEM) * NT_SMEM +
                                  warp * 32 + (e & 31);
-            const Y4 r = slow_point(&g, smem, __ldg(x + ps), load_scale<Q_IS_Q>(q2 + ps), lane8);
-            store4(out, out_stride, ps, row, odd, r.E, r.O);  // the gather ran on THIS lane: its parity
+            const YW<W> r = slow_point<W>(&g, smem, __ldg(x + ps), load_scale<Q_IS_Q>(q2 + ps), lane8);
+            store_cols<W>(out, out_stride, ps, row, r.v);
         }
         __syncwarp();
     };
@@ -414,8 +463,6 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         if (any_in) {
             // ---- locate (LUT guess + exact comparisons where needed), weights, one gather per point.
             // A lane whose point is out of range computes a dummy in-range point and stores nothing.
-            Win w[PPT_SMEM];
-            double vw[PPT_SMEM][4];
 #pragma unroll
             for (int k = 0; k < PPT_SMEM; k++) {
                 const double xs = in_range[k] ? xv[k] : g.x_min, qs = in_range[k] ? qv[k] : g.q2_min;
@@ -424,16 +471,19 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                 const int gi = locate_q(g, sv, qs, v);
                 const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
                 const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
-                double wu[4];
+                double wu[4], vw[4], y[W];
                 weights_rec32(rx, (u - rx.z0) * rx.inv_dz, wu);
-                weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vw[k]);
-                make_win(w[k], tab + (uint32_t)((gi - 1) * (int)RB), i - 1, wu, lane8);
-            }
-#pragma unroll
-            for (int k = 0; k < PPT_SMEM; k++) {
-                double2 E, O;
-                gather4(w[k], vw[k], rb1, rb2, rb3, E, O);
-                if (in_range[k]) store4(out, out_stride, p0 + k * NT_SMEM, row, odd, E, O);
+                weights_rec32(rq, (v - rq.z0) * rq.inv_dz, vw);
+                if (W == 4) {  // written out: the register allocation of this path is at the 128 cap
+                    Win w;
+                    make_win(w, tab + (uint32_t)((gi - 1) * (int)RB), i - 1, wu, lane8);
+                    double2 E, O;
+                    gather4(w, vw, RB, rb2, rb3, E, O);
+                    y[0] = odd ? O.x : E.x; y[1] = odd ? O.y : E.y; y[W - 2] = odd ? E.x : O.x; y[W - 1] = odd ? E.y : O.y;
+                } else {
+                    eval_stencil<W>(tab, RB, rb2, rb3, gi - 1, i - 1, wu, vw, lane8, y);
+                }
+                if (in_range[k]) store_cols<W>(out, out_stride, p0 + k * NT_SMEM, row, y);
             }
         }
 #pragma unroll
@@ -444,7 +494,10 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const bool slow = live && !in_range[k] && !invalid;
             const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
             if (invalid) {
-                store4(out, out_stride, p, row, false, make_double2(qnan, qnan), make_double2(qnan, qnan));
+                double nanv[W];
+#pragma unroll
+                for (int c = 0; c < W; c++) nanv[c] = qnan;
+                store_cols<W>(out, out_stride, p, row, nanv);
                 if (job == 0) atomicAdd(g.n_invalid, 1ULL);
             }
             if (slow_mask) {  // warp-uniform: append the out-of-grid points to their class lists
@@ -472,41 +525,46 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         if ((cnts >> (6 * c)) & 63) flush(c, (cnts >> (6 * c)) & 63);
 }
 
-static int smem_needed(const GridDev &d) { return d.pre_bytes + d.slice_bytes + d.post_bytes; }
+static int smem_needed(const GridDev &d, int W) { return d.pre_bytes + (W == 4 ? d.slice_bytes : d.slice2_bytes) + d.post_bytes; }
 static const int STATIC_SMEM = 256;  // >= the kernel's static shared memory (mbarrier)
 
+// bit 0: the 4-column slices fit the device's shared memory, bit 1: the 2-column slices do
 int pdfb_smem_eligible(const pdfb_grid *g)
 {
     if (getenv("PDFB_FORCE_FALLBACK")) return 0;  // testing: force the read-only-cache path
     int dev_max = 0;
     if (cudaDeviceGetAttribute(&dev_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, g->device) != cudaSuccess) return 0;
-    if (smem_needed(g->d) + STATIC_SMEM > dev_max) return 0;
+    int ok = 0;
+    if (smem_needed(g->d, 4) + STATIC_SMEM <= dev_max && !getenv("PDFB_NO_W4")) ok |= 1;  // (testing: 2-column path only)
+    if (smem_needed(g->d, 2) + STATIC_SMEM <= dev_max) ok |= 2;
+    if (!ok) return 0;
     // the attribute is per function, not per handle: raise it once to the device maximum
     static int attr_set_for = -1;
     if (attr_set_for != g->device) {
-        if (cudaFuncSetAttribute(k_xfxq2_smem<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - STATIC_SMEM) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfxq2_smem<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, dev_max - STATIC_SMEM) != cudaSuccess) {
+        const int lim = dev_max - STATIC_SMEM;
+        if (cudaFuncSetAttribute(k_xfxq2_smem<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
+            cudaFuncSetAttribute(k_xfxq2_smem<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
+            cudaFuncSetAttribute(k_xfxq2_smem<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
+            cudaFuncSetAttribute(k_xfxq2_smem<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess) {
             cudaGetLastError();
             return 0;
         }
         attr_set_for = g->device;
     }
-    return 1;
+    return ok;
 }
 
-int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
-                           int member0, int n_mem)
+// passes of a request on W-column groups: one per (group, distinct use of its columns); a PID asked
+// for twice gets an extra pass
+static int build_passes(int W, int n_groups, int n_req, const int *cols, PassList &pl)
 {
-    // passes: one per (flavour group, distinct use of its columns); duplicates get extra passes
-    PassList pl;
     pl.n = 0;
     bool used[PDFB_MAX_PIDS] = {false};
     for (int left = n_req; left > 0;) {
-        for (int grp = 0; grp < g->d.n_groups && left > 0; grp++) {
+        for (int grp = 0; grp < n_groups && left > 0; grp++) {
             int row[4] = {-1, -1, -1, -1}, hit = 0;
             for (int r = 0; r < n_req; r++)
-                if (!used[r] && cols[r] / 4 == grp && row[cols[r] & 3] < 0) { row[cols[r] & 3] = r; used[r] = true; hit++; }
+                if (!used[r] && cols[r] / W == grp && row[cols[r] % W] < 0) { row[cols[r] % W] = r; used[r] = true; hit++; }
             if (!hit) continue;
             if (pl.n >= PDFB_MAX_PIDS) return PDFB_ELIMIT;
             pl.group[pl.n] = grp;
@@ -515,6 +573,25 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
             left -= hit;
         }
     }
+    return PDFB_OK;
+}
+
+int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
+                           int member0, int n_mem)
+{
+    // Width: a 4-column pass costs ~5.6 shared-memory wavefronts per point (4 gather + 1.6 setup and
+    // I/O), a 2-column pass ~3.6; take the cheaper plan among the widths that fit shared memory.
+    PassList pl4, pl2;
+    pl4.n = pl2.n = 0;
+    const int ok = g->d.smem_ok;
+    int rc = PDFB_OK;
+    if (ok & 1) rc = build_passes(4, g->d.n_groups, n_req, cols, pl4);
+    if (!rc && (ok & 2)) rc = build_passes(2, g->d.n_groups2, n_req, cols, pl2);
+    if (rc) return rc;
+    const bool use2 = !(ok & 1) || ((ok & 2) && 3.6 * pl2.n < 5.6 * pl4.n);
+    const PassList &pl = use2 ? pl2 : pl4;
+    const int W = use2 ? 2 : 4;
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
     // jobs = (member, pass).  Few jobs: the SMs are split between them and each CTA is persistent
@@ -527,10 +604,11 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     long long tiles = (n + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
     if (per_job > tiles) per_job = (int)tiles;
     const unsigned grid = (unsigned)(per_job * n_jobs);
-    if (q_is_q)
-        k_xfxq2_smem<true><<<grid, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride, member0, n_req, (int)n_jobs);
-    else
-        k_xfxq2_smem<false><<<grid, NT_SMEM, smem_needed(g->d), st>>>(g->d, pl, n, x, q2, out, out_stride, member0, n_req, (int)n_jobs);
+    const int smem = smem_needed(g->d, W);
+#define PDFB_LAUNCH(Q, WW) k_xfxq2_smem<Q, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, n, x, q2, out, out_stride, member0, n_req, (int)n_jobs)
+    if (W == 4) { if (q_is_q) PDFB_LAUNCH(true, 4); else PDFB_LAUNCH(false, 4); }
+    else        { if (q_is_q) PDFB_LAUNCH(true, 2); else PDFB_LAUNCH(false, 2); }
+#undef PDFB_LAUNCH
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

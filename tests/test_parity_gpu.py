@@ -394,10 +394,49 @@ def test_pdf_object_api(torch_cuda, tmp_path):
         check_parity(a.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what="PDF.xfxQ2")
         allm = pdf.xfxQ2(None, x, q2, members=(0, 2))
         assert allm.shape == (2, 13, len(x))
-        assert torch.equal(allm[0, 12], a[0])                         # PID 21 is the last of PIDS_13
+        # PID 21 is the last of PIDS_13 (2-column plan for the pair, 4-column plan for all 13: same
+        # numbers up to summation order)
+        assert torch.allclose(allm[0, 12], a[0], rtol=1e-11, atol=1e-14)
         assert torch.equal(pdf.xfxQ(None, x, q, members=(0, 2)), pdf.xfxQ2(None, x, q * q, members=(0, 2)))
         assert torch.equal(pdf.xfxQ([2], x, q), pdf.xfxQ2([2], x, q * q))
         al = pdf.alphasQ2(q2)
         check_parity(al.cpu().numpy(), oracle.OracleAlphas.from_spec(aspec).q2(q2), what="PDF.alphasQ2")
         assert torch.equal(pdf.alphasQ(q), pdf.alphasQ2(q * q)) and torch.equal(al, pdf2.alphasQ2(q2))
         assert pdf.n_invalid() == 0
+
+
+def test_two_column_slices(torch_cuda, grid2, ograph2, monkeypatch):
+    """The 2-column shared-memory path (row pairs as one 8-chunk run): (a) forced for every request
+    on the NNPDF-shaped grid, (b) chosen by itself for one- and two-flavour requests, (c) the only
+    shared-memory path of a grid whose 4-column slice does not fit (150 x 50 knots)."""
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    x, q2 = W.queries_extrapolation_mix(grid2, 40_003)
+    xs, qs = W.scan_points(grid2, per_cell=2)
+    x, q2 = np.concatenate([x, xs]), np.concatenate([q2, qs])
+    ref, sc = ograph2.xfxq2(pids, x, q2, with_scale=True)
+    monkeypatch.setenv("PDFB_NO_W4", "1")
+    h = B.load_pdf_spec(grid2)
+    monkeypatch.delenv("PDFB_NO_W4")
+    assert B.pdf_grid_uses_smem_path(h)
+    check_parity(gpu_xfxq2(torch, h, pids, x, q2), ref, sc, max_clause_frac=5e-3, what="2-column path, 11 flavours")
+    sub = [21, 21, -5, 3]
+    rs, ss = ograph2.xfxq2(sub, x, q2, with_scale=True)
+    check_parity(gpu_xfxq2(torch, h, sub, x, q2), rs, ss, max_clause_frac=5e-3, what="2-column path, duplicates")
+    B.pdf_grid_free(h)
+    # (b) default handle: narrow requests take the 2-column plan, same numbers within tolerance
+    h = B.load_pdf_spec(grid2)
+    for req in ([21], [4, 5], [-5]):
+        r1, s1 = ograph2.xfxq2(req, x, q2, with_scale=True)
+        check_parity(gpu_xfxq2(torch, h, req, x, q2), r1, s1, max_clause_frac=5e-3, what=f"narrow request {req}")
+    B.pdf_grid_free(h)
+    # (c) a grid too large for 4-column slices
+    big = W.make_pdf_grid(1e-9, 1.0, 150, (1.65, 4.92, 172.5, 1.0e5), (10, 20, 20), W.PIDS_11)
+    hb = B.load_pdf_spec(big)
+    assert B.pdf_grid_uses_smem_path(hb)
+    xb, qb = W.queries_extrapolation_mix(big, 30_011)
+    xs, qs = W.scan_points(big, per_cell=1)
+    xb, qb = np.concatenate([xb, xs]), np.concatenate([qb, qs])
+    rb, sb = oracle.OraclePdfGrid.from_spec(big).xfxq2(pids, xb, qb, with_scale=True)
+    check_parity(gpu_xfxq2(torch, hb, pids, xb, qb), rb, sb, max_clause_frac=5e-3, what="150 x 50 grid")
+    B.pdf_grid_free(hb)
