@@ -60,6 +60,9 @@ __device__ __noinline__ double cont_e(double r, double yL, double yH)  // readin
     return fma(r, yH - yL, yL);
 }
 
+// the coordinate logarithm of the out-of-grid path: pdfb_ln, one copy (code size, see cont_e)
+__device__ __noinline__ double ln_slow(double a) { return pdfb_ln(a); }
+
 // rule C (reading O5): y0 * rho^(gamma*rho + 1 - rho), gamma from the probe at 1.01 q_min
 __device__ __noinline__ double rule_c(double y0, double y1, double rho)
 {
@@ -288,20 +291,20 @@ __device__ __noinline__ YW<W> slow_point(const GridDev *gp, unsigned char *smem,
     int node0 = 0;
     double rA = 0.0;
     if (!low_x) {
-        const double u = ln_pos(xv);
+        const double u = ln_slow(xv);
         const int i = locate_x(g, sv, xv, u);
         const IntervalRec32 r = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
         weights_rec32(r, (u - r.z0) * r.inv_dz, wu1);
         node0 = i - 1;
     } else {
-        rA = (pdfb_ln(xv) - g.U0) * g.inv_dU01;
+        rA = (ln_slow(xv) - g.U0) * g.inv_dU01;
     }
     // ---- rows: one stencil in range, else two probes (rules B, C); row = table row of stencil row 0
     int row1, row2;
     double vw1[4], vw2[4];
     double rB = 0.0;
     if (high_q) {  // the last two Q^2 knots of the last sub-grid
-        rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
+        rB = (ln_slow(qv) - g.Va) * g.inv_dVab;
         row1 = row2 = g.nq_tot - 4;
         vw1[0] = vw1[1] = vw1[3] = 0.0; vw1[2] = 1.0;
         vw2[0] = vw2[1] = vw2[2] = 0.0; vw2[3] = 1.0;
@@ -312,7 +315,7 @@ __device__ __noinline__ YW<W> slow_point(const GridDev *gp, unsigned char *smem,
 #pragma unroll
         for (int b = 0; b < 4; b++) vw2[b] = g.wvC[b];
     } else {
-        const double v = ln_pos(qv);
+        const double v = ln_slow(qv);
         const int gi = locate_q(g, sv, qv, v);
         const IntervalRec32 r = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
         weights_rec32(r, (v - r.z0) * r.inv_dz, vw1);
