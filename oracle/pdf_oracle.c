@@ -22,7 +22,8 @@
  * in interior cells only, scipy CubicHermiteSpline special case, threshold side rule,
  * continuity and power-law exactness of the continuation, one-loop alpha_s closed form.
  * PARITY UNPINNED (no source in the paper, no LHAPDF here to compare with): the
- * continuation constants of O4/O5 (1e-3, 1e-5, -2.5, 1.01, 0.01) and reading Q10
+ * continuation constants of O4/O5 (1e-3, 1e-5, -2.5, 1.01, 0.01, gamma = 1 for |y0| < 1e-5)
+ * and reading Q10
  * (alpha_s frozen below the first node).
  *
  * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC pdf_oracle.c -lquadmath -lm
@@ -195,7 +196,8 @@ static double o3(const ogrid *g, int k, double x, double q2)
 
 /* ------------------------------------------------------------------ O4, O5 */
 #define CONT_LOGLOG_MIN 1e-3 /* O4: both values above this -> linear in log-log      */
-#define LOWQ_Y0_MIN 1e-5     /* O5-C: |y0| below this -> anomalous dimension gamma=0 */
+#define LOWQ_Y0_MIN 1e-5     /* O5-C: |y0| below this -> gamma = LOWQ_GAMMA_SMALL     */
+#define LOWQ_GAMMA_SMALL 1.0 /* O5-C: then xf = y0 * rho, linear in Q^2 (reading Q9) */
 #define LOWQ_GAMMA_MIN -2.5  /* O5-C: gamma clamp                                    */
 #define LOWQ_PROBE 1.01      /* O5-C: second probe at 1.01 q_min                     */
 #define LOWQ_PROBE_STEP 0.01
@@ -235,7 +237,7 @@ static double rule_c(const ogrid *g, int k, double x, double q2)
 {
     double qmin = g->q2[0];
     double y0 = G(g, k, x, qmin), y1 = G(g, k, x, LOWQ_PROBE * qmin);
-    double gamma = 0.0;
+    double gamma = LOWQ_GAMMA_SMALL;
     if (fabs(y0) >= LOWQ_Y0_MIN) gamma = fmax(LOWQ_GAMMA_MIN, (y1 - y0) / y0 / LOWQ_PROBE_STEP);
     double rho = q2 / qmin;
     return y0 * pow(rho, gamma * rho + 1.0 - rho);
@@ -329,7 +331,7 @@ static double xf_scale(const ogrid *g, int k, double x, double q2)
     if (q2 < qmin) {
         double y0 = G(g, k, x, qmin), y1 = G(g, k, x, LOWQ_PROBE * qmin);
         double s0 = G_scale(g, k, x, qmin), s1 = G_scale(g, k, x, LOWQ_PROBE * qmin);
-        double rho = q2 / qmin, gamma = 0.0, dg0 = 0.0, dg1 = 0.0;
+        double rho = q2 / qmin, gamma = LOWQ_GAMMA_SMALL, dg0 = 0.0, dg1 = 0.0;
         if (fabs(y0) >= LOWQ_Y0_MIN) {
             double graw = (y1 - y0) / y0 / LOWQ_PROBE_STEP;
             gamma = fmax(LOWQ_GAMMA_MIN, graw);

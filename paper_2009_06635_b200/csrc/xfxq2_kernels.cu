@@ -154,7 +154,7 @@ k_xfxq2_v0(GridDev g, ReqCols rc, long long n, const double *__restrict__ x, con
         if (high_q) {
             res = continuation(rB, y1, y2);
         } else if (low_q) {  // rule C: y0 * rho^(gamma*rho + 1 - rho)
-            double gamma = 0.0;
+            double gamma = 1.0;  // |y0| < 1e-5: y0 * rho (reading Q9)
             if (fabs(y1) >= 1e-5) gamma = fmax(-2.5, (y2 - y1) / y1 / 0.01);
             res = y1 * pow(rho, fma(gamma, rho, 1.0 - rho));
         }

@@ -63,10 +63,11 @@ __device__ __noinline__ double cont_e(double r, double yL, double yH)  // readin
 // the coordinate logarithm of the out-of-grid path: pdfb_ln, one copy (code size, see cont_e)
 __device__ __noinline__ double ln_slow(double a) { return pdfb_ln(a); }
 
-// rule C (reading O5): y0 * rho^(gamma*rho + 1 - rho), gamma from the probe at 1.01 q_min
+// rule C (reading O5): y0 * rho^(gamma*rho + 1 - rho), gamma from the probe at 1.01 q_min;
+// |y0| < 1e-5: gamma = 1, i.e. y0 * rho (reading Q9)
 __device__ __noinline__ double rule_c(double y0, double y1, double rho)
 {
-    double gamma = 0.0;
+    double gamma = 1.0;
     if (fabs(y0) >= 1e-5) gamma = fmax(-2.5, (y1 - y0) / y0 / 0.01);
     return y0 * pow(rho, fma(gamma, rho, 1.0 - rho));
 }

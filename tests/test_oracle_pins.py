@@ -392,13 +392,72 @@ def test_I8_rule_C_limits_clamp_and_fallback():
     assert abs(y0) > 1e-5 and (y1 - y0) / y0 / 0.01 < -2.6
     f = og2.xfxq2([21], [x], [0.5 * qmin])[0, 0]
     assert np.isclose(f, y0 * 0.5 ** (-2.5 * 0.5 + 0.5), rtol=1e-13)
-    # (v) |y0| < 1e-5 -> gamma = 0
+    # (v) |y0| < 1e-5 -> gamma = 1: the exponent gamma*rho + 1 - rho is 1 for every rho, so xf is
+    # the straight line y0 * Q^2/q_min through the origin -- the limit (ii) that the regular branch
+    # reaches as rho -> 0, now at every rho (reading Q9)
     spec3, _ = _powerlaw_spec(A=1e-6, g=0.4)
     og3 = oracle.OraclePdfGrid.from_spec(spec3)
     y0 = og3.xfxq2([21], [0.5], [qmin])[0, 0]
-    assert abs(y0) < 1e-5
-    f = og3.xfxq2([21], [0.5], [0.5 * qmin])[0, 0]
-    assert np.isclose(f, y0 * 0.5 ** 0.5, rtol=1e-13)
+    assert 0 < abs(y0) < 1e-5
+    rhos = np.array([0.9, 0.5, 0.1, 1e-3])
+    f = og3.xfxq2([21], np.full_like(rhos, 0.5), rhos * qmin)[0]
+    assert np.allclose(f, y0 * rhos, rtol=2e-15, atol=0)
+    assert np.allclose(np.diff(f) / np.diff(rhos), y0, rtol=1e-12)  # one slope: a straight line
+
+
+def _two_column_spec(yL, yH, qk=None):
+    """Grid constant along Q whose first two x columns hold yL, yH (values given explicitly)."""
+    xk = np.geomspace(1e-4, 1.0, 7)
+    qk = np.geomspace(2.0, 100.0, 6) if qk is None else qk
+    col = np.array([yL, yH, 0.5, 0.4, 0.3, 0.2, 0.0])
+    vals = np.repeat(col[:, None], len(qk), axis=1)[:, :, None]
+    return make_spec(xk, [qk], [21], values=[vals])
+
+
+@pytest.mark.parametrize("yL,loglog", [(1.001e-3, True), (0.999e-3, False), (1e-3, False)])
+def test_I8_O4_switches_at_1e_minus_3(yL, loglog):
+    """O4 is linear in log-log iff BOTH values are strictly above 1e-3, else linear in log-lin:
+    pinned 0.1 % either side of the switch and exactly on it (closed forms written out here)."""
+    yH = 1.3e-3
+    spec = _two_column_spec(yL, yH)
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    x0, x1 = spec.x_knots[0], spec.x_knots[1]
+    q2 = float(spec.q_knots[2]) ** 2          # on a Q^2 knot: the two probes are yL, yH exactly
+    xs = x0 * np.array([0.5, 1e-2, 1e-6])
+    r = np.log(xs / x0) / np.log(x1 / x0)
+    got = og.xfxq2([21], xs, np.full_like(xs, q2))[0]
+    power = yL * (yH / yL) ** r
+    line = yL + r * (yH - yL)
+    assert np.all(np.abs(power - line) > 1e-6)  # the two branches are far apart at these points
+    assert np.allclose(got, power if loglog else line, rtol=1e-13, atol=0)
+    # the same switch with the roles swapped (yH at the threshold)
+    spec = _two_column_spec(1.3e-3, yL)
+    got = oracle.OraclePdfGrid.from_spec(spec).xfxq2([21], xs, np.full_like(xs, q2))[0]
+    power, line = 1.3e-3 * (yL / 1.3e-3) ** r, 1.3e-3 + r * (yL - 1.3e-3)
+    assert np.allclose(got, power if loglog else line, rtol=1e-13, atol=0)
+
+
+@pytest.mark.parametrize("y0,regular", [(1.001e-5, True), (0.999e-5, False), (1e-5, True), (-1.001e-5, True), (-0.999e-5, False)])
+def test_I8_O5C_fallback_switches_at_1e_minus_5(y0, regular):
+    """Rule C takes gamma from the probe at 1.01 q_min iff |y0| >= 1e-5, else gamma = 1."""
+    xk = np.geomspace(1e-4, 1.0, 7)
+    qk = np.geomspace(2.0, 100.0, 6)
+    g = 0.3
+    row = (qk * qk / qk[0] ** 2) ** g
+    vals = np.empty((len(xk), len(qk), 1))
+    vals[:, :, 0] = y0 * row[None, :]
+    vals[:, 0, 0] = y0                      # the q_min row holds y0 exactly
+    spec = make_spec(xk, [qk], [21], values=[vals])
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    x, qmin = float(xk[3]), spec.q2_min
+    assert og.xfxq2([21], [x], [qmin])[0, 0] == y0
+    y1 = og.xfxq2([21], [x], [1.01 * qmin])[0, 0]
+    gamma = max(-2.5, (y1 - y0) / y0 / 0.01)
+    assert 0.2 < gamma < 0.4                # far from 1: the two branches differ visibly
+    rho = np.array([0.8, 0.3, 0.05])
+    got = og.xfxq2([21], np.full_like(rho, x), rho * qmin)[0]
+    want = y0 * rho ** (gamma * rho + 1 - rho) if regular else y0 * rho
+    assert np.allclose(got, want, rtol=1e-13, atol=0)
 
 
 def test_invalid_points_give_nan_and_are_counted(grid1):
@@ -510,6 +569,45 @@ def test_scale_bounds_weighted_stencil_sum():
         S = np.abs(wu) @ np.abs(spec.sub_values(s)[:, :, 0]) @ np.abs(wv)
         assert sc >= S * (1 - 1e-12) and sc <= 8 * S + 1e-300
         assert abs(o) <= sc * (1 + 1e-12)
+
+
+@pytest.mark.parametrize("kind", ["loglog", "loglin", "tiny"])
+def test_scale_bounds_the_sensitivity_outside_the_grid(kind):
+    """The scale helper outside the grid (cont_scale, G_scale, the Q^2 < q_min and Q^2 > q_max
+    branches of xf_scale) against what it claims to bound: S = sum_knots |d result / d f_knot| |f_knot|,
+    the derivatives taken numerically by perturbing one table value at a time.  Classes A, B, C
+    and both corners; grids whose values take O4's log-log branch, its log-lin branch, and rule C's
+    |y0| < 1e-5 branch."""
+    rng = np.random.default_rng(11 if kind == "loglog" else 12)
+    xk = rand_knots(rng, 1e-4, 1.0, 5)
+    subs = [rand_knots(rng, 1.5, 9.0, 4), rand_knots(rng, 9.0, 200.0, 4)]
+    if kind == "loglog":   # all values >> 1e-3
+        values = [np.exp(0.3 * rng.normal(size=(len(xk), len(q), 1))) for q in subs]
+    else:                  # all |values| < 1e-3, both signs; "tiny": |y0| < 1e-5, rule C's gamma = 1 branch
+        amp = 2e-4 if kind == "loglin" else 2e-6
+        values = [amp * rng.normal(size=(len(xk), len(q), 1)) for q in subs]
+    spec = make_spec(xk, subs, [21], values=values)
+    x0, xm = spec.x_knots[0], 0.37 * spec.x_knots[2] + 0.63 * spec.x_knots[3]
+    qlo, qhi, qmid = spec.q2_min, spec.q2_max, 30.0
+    pts = np.array([(0.3 * x0, qmid), (1e-3 * x0, 4.0),          # A
+                    (xm, 3.0 * qhi), (xm, 1e3 * qhi),            # B
+                    (xm, 0.6 * qlo), (xm, 0.05 * qlo),           # C
+                    (0.2 * x0, 7.0 * qhi), (0.2 * x0, 0.4 * qlo)])  # corners A+B, A+C
+    x, q2 = pts[:, 0].copy(), pts[:, 1].copy()
+    base, scale = oracle.OraclePdfGrid.from_spec(spec).xfxq2([21], x, q2, with_scale=True)
+    flat = spec.values.copy()
+    S = np.zeros(len(x))
+    for e in range(len(flat)):
+        d = 1e-6 * abs(flat[e])
+        hi, lo = flat.copy(), flat.copy()
+        hi[e] += d; lo[e] -= d
+        fh = oracle.OraclePdfGrid(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, hi).xfxq2([21], x, q2)[0]
+        fl = oracle.OraclePdfGrid(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, lo).xfxq2([21], x, q2)[0]
+        S += np.abs(fh - fl) / (2 * d) * abs(flat[e])
+    assert np.all(S > 0)
+    assert np.all(scale[0] >= S * (1 - 1e-6)), (scale[0] / S)
+    assert np.all(scale[0] <= 400 * S), (scale[0] / S)   # a bound, not a blank cheque
+    assert np.all(np.abs(base[0]) <= scale[0] * (1 + 1e-12))
 
 
 # ----------------------------------------------------------------------------------
