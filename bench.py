@@ -103,6 +103,22 @@ def cpu_baseline(grid, x, q2, pids, target_s=12.0):
             "sample": f"first {m} points of the config-3 batch x {len(pids)} flavours, {dt:.1f} s"}
 
 
+def parity_population(torch, out_d, grid, x_h, q2_h, pids, chunk=10_000_000):
+    """--parity: EVERY output of the timed batch against the oracle ("parity is
+    checked on all points", config 3 in 1e7-point chunks): max eq.-1 difference,
+    outputs breaking the 1e-12 / 1e-15 rule, outputs that needed the conditioning clause."""
+    import oracle
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from parity_util import check_parity_population
+    og = oracle.OraclePdfGrid.from_spec(grid)
+    t = time.perf_counter()
+    st = check_parity_population(lambda a, b: out_d[:, a:b].cpu().numpy(), og, pids, x_h, q2_h, chunk=chunk,
+                                 max_clause_frac=2e-3, what="bench --parity, config 3 all points")
+    st["seconds"] = time.perf_counter() - t
+    st["rule"] = "|d| <= 1e-12 |ref|, or |d| <= 1e-15 where |ref| < 1e-3; clause |d| <= 1e-12 S (DESIGN.md 5)"
+    return st
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on the box's host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -353,6 +369,10 @@ def run_gpu(args):
         line["multi_member"] = bench_members(torch, B, local, args.members)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(grid, x_h, q2_h, pids)
+    if args.parity:
+        step()
+        torch.cuda.synchronize()
+        line["parity"] = parity_population(torch, out_d, grid, x_h, q2_h, pids)
     B.pdf_grid_free(h)
     if dist is not None:
         dist.destroy_process_group()
@@ -368,6 +388,7 @@ def main():
     ap.add_argument("--points", type=int, default=N_FULL, help="points per GPU (config 3: 1e8)")
     ap.add_argument("--e2e-points", type=int, default=N_FULL)
     ap.add_argument("--ref-points", type=int, default=2_000_000, help="oracle sample per step")
+    ap.add_argument("--parity", action="store_true", help="check every output of the batch against the oracle (~2 min)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-members", action="store_true")

@@ -1,6 +1,10 @@
 """Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (one
-pdf_xfxq2 call over the whole batch): sampled outputs against the oracle, plus properties that
-hold at any size (no NaN in range, every output written, invalid counter zero)."""
+pdf_xfxq2 call over the whole batch).  Configs 2, 4 and 5: EVERY output against the oracle
+("parity is checked on all points"), the oracle run in chunks and its scale helper
+only where the 1e-12 / 1e-15 rule breaks; the totals (max eq. 1 difference, rule
+violations, clause uses) go to the parity log.  Config 3 (1e8 points): sampled outputs plus
+properties that hold at any size here; its full population is `bench.py --parity` (~2 min of
+oracle), which puts the same totals into the bench line."""
 import numpy as np
 import pytest
 
@@ -8,7 +12,7 @@ pytestmark = pytest.mark.gpu
 
 import oracle
 from paper_2009_06635_b200 import binding as B, build, workloads as W
-from parity_util import check_parity
+from parity_util import check_parity, check_parity_population
 
 
 @pytest.fixture(scope="module")
@@ -30,15 +34,20 @@ def _run(torch, h, pids, x, q2):
     return out
 
 
-def _sample_check(torch, out, og, pids, x, q2, m, what, frac=2e-3):
-    n = len(x)
-    idx = np.unique(np.concatenate([np.random.default_rng(99).integers(0, n, m),
-                                    np.arange(0, 4096), np.arange(n - 4096, n)]))
-    got = out[:, torch.from_numpy(idx).cuda()].cpu().numpy()
-    ref, sc = og.xfxq2(pids, x[idx], q2[idx], with_scale=True)
-    st = check_parity(got, ref, sc, max_clause_frac=frac, what=what)
+def _population(torch, out, og, pids, x, q2, what, frac):
+    st = check_parity_population(lambda a, b: out[:, a:b].cpu().numpy(), og, pids, x, q2,
+                                 chunk=2_000_000, max_clause_frac=frac, what=what)
     print(what, st)
     return st
+
+
+def test_config2_all_1e6_points(env, grid2):
+    torch, h, og = env
+    x, q2 = W.queries_in_range(grid2, 1_000_000, 2)
+    pids = list(W.PIDS_11)
+    out = _run(torch, h, pids, x, q2)
+    st = _population(torch, out, og, pids, x, q2, "config2 all points", 2e-3)
+    assert st["n"] == 11_000_000 and B.pdf_grid_status(h) == 0
 
 
 def test_config3_1e8_points_11_flavours(env, grid2):
@@ -49,35 +58,42 @@ def test_config3_1e8_points_11_flavours(env, grid2):
     out = _run(torch, h, pids, x, q2)
     assert not bool(torch.isnan(out).any())          # every output written, none NaN in range
     assert B.pdf_grid_status(h) == 0
-    _sample_check(torch, out, og, pids, x, q2, 300_000, "config3 full size")
+    idx = np.unique(np.concatenate([np.random.default_rng(99).integers(0, n, 1_000_000),
+                                    np.arange(0, 4096), np.arange(n - 4096, n)]))
+    got = out[:, torch.from_numpy(idx).cuda()].cpu().numpy()
+    xi, qi = x[idx], q2[idx]
+    st = check_parity(got, og.xfxq2(pids, xi, qi), lambda c: og.xfxq2(pids, xi[c], qi[c], with_scale=True)[1],
+                      what="config3 full size, 1e6-point sample")
+    print("config3", st)
     del out
     torch.cuda.empty_cache()
 
 
 @pytest.mark.parametrize("pids", [[21], list(W.PIDS_11)])
-def test_config4_1e7_points(env, grid2, pids):
+def test_config4_all_1e7_points(env, grid2, pids):
     torch, h, og = env
     x, q2 = W.queries_extrapolation_mix(grid2, 10_000_000)
     out = _run(torch, h, pids, x, q2)
     assert not bool(torch.isnan(out).any())
-    _sample_check(torch, out, og, pids, x, q2, 200_000, f"config4 full size F={len(pids)}", frac=5e-3)
+    st = _population(torch, out, og, pids, x, q2, f"config4 all points F={len(pids)}", 5e-3)
+    assert st["n"] == 10_000_000 * len(pids)
 
 
-def test_config5_1e7_events(env, grid2):
+def test_config5_all_1e7_events(env, grid2):
     torch, h, og = env
     x1, x2, q2 = W.queries_mc_events(grid2, 10_000_000)
     pids = list(W.PIDS_11)
-    for x in (x1, x2):
+    for name, x in (("x1", x1), ("x2", x2)):
         out = _run(torch, h, pids, x, q2)
         assert not bool(torch.isnan(out).any())
-        _sample_check(torch, out, og, pids, x, q2, 100_000, "config5 full size")
+        _population(torch, out, og, pids, x, q2, f"config5 all events, {name}", 2e-3)
+        del out
     aspec = W.make_alphas_grid()
     ha = B.load_alphas_spec(aspec)
     dq = torch.from_numpy(q2).cuda()
     a = torch.empty_like(dq)
     B.alphas_q2(ha, dq, a)
     torch.cuda.synchronize()
-    idx = np.random.default_rng(5).integers(0, len(q2), 200_000)
-    check_parity(a[torch.from_numpy(idx).cuda()].cpu().numpy(), oracle.OracleAlphas.from_spec(aspec).q2(q2[idx]),
-                 what="config5 alphas full size")
+    st = check_parity(a.cpu().numpy(), oracle.OracleAlphas.from_spec(aspec).q2(q2), what="config5 alphas, all events")
+    assert st["n"] == 10_000_000 and st["n_clause"] == 0
     B.alphas_grid_free(ha)

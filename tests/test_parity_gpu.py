@@ -187,7 +187,7 @@ def test_tiny_subgrids_two_and_three_knots(torch_cuda):
     h = B.load_pdf_spec(spec)
     x, q2 = W.scan_points(spec, per_cell=5)
     ref, sc = og.xfxq2([1, 21], x, q2, with_scale=True)
-    check_parity(gpu_xfxq2(torch_cuda, h, [1, 21], x, q2), ref, sc, max_clause_frac=1.0, what="tiny")
+    check_parity(gpu_xfxq2(torch_cuda, h, [1, 21], x, q2), ref, sc, what="tiny")  # measured: no output needs the clause
     B.pdf_grid_free(h)
 
 
@@ -231,7 +231,7 @@ def test_irregular_grid_on_the_smem_path(torch_cuda):
     x, q2 = np.concatenate([x, xo]), np.concatenate([q2, qo])
     for req in ([21], [0, 22], [4, -3, 1], pids_all, [2, 2, 21, -1, 3, 22, 2]):
         ref, sc = og.xfxq2(req, x, q2, with_scale=True)
-        check_parity(gpu_xfxq2(torch_cuda, h, req, x, q2), ref, sc, max_clause_frac=1.0, what=f"irregular {req}", clause_rel=4e-12)
+        check_parity(gpu_xfxq2(torch_cuda, h, req, x, q2), ref, sc, max_clause_frac=4e-4, what=f"irregular {req}", clause_rel=4e-12)  # measured 1.2e-4 .. 1.5e-4 of the outputs (parity log)
     B.pdf_grid_free(h)
 
 
@@ -329,7 +329,7 @@ def test_member_set(torch_cuda):
     B.pdf_xfxq2_members(ht, 1, 3, [21, 1], torch.from_numpy(xs).cuda(), torch.from_numpy(qs).cuda(), ot)
     torch.cuda.synchronize()
     rt, st = oracle.xfxq2_members(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tv[1:4], [21, 1], xs, qs, with_scale=True)
-    check_parity(ot.cpu().numpy(), rt, st, max_clause_frac=1.0, what="tiny member set")
+    check_parity(ot.cpu().numpy(), rt, st, what="tiny member set")
     B.pdf_grid_free(ht)
 
 

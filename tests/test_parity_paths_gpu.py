@@ -1,0 +1,154 @@
+"""GPU parity of the paths the main parity file does not reach ("parity coverage
+holes"): the general alpha_s kernel (> 192 nodes), alphas_q2_host, the read-only-cache kernel
+k_xfxq2_v0 forced on the NNPDF-shaped grid, and rule C's small-|y0| branch."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+import oracle
+from paper_2009_06635_b200 import binding as B, build, workloads as W
+from parity_util import check_parity
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    build.build()
+    B.lib()
+    return torch
+
+
+def _alphas_points(aspec, rng, n):
+    k2 = aspec.q_knots ** 2
+    return np.concatenate([k2, np.nextafter(k2, 0), np.nextafter(k2, np.inf),
+                           np.exp(rng.uniform(np.log(0.1), np.log(1e12), n)), [0.0, -1.0, np.nan, np.inf]])
+
+
+def test_alphas_general_kernel_300_nodes(torch_cuda):
+    """A 300-node list (> 192: k_alphas, binary search + weights4, not the replicated-line fast
+    path), with discontinuities at the thresholds; nodes, their neighbours, outside, invalid."""
+    torch = torch_cuda
+    aspec = W.make_alphas_grid(nq_per_sub=(20, 40, 100, 140), jump=(1.0, 1.02, 1.0404, 1.061208))
+    assert len(aspec.q_knots) == 300
+    ha = B.load_alphas_spec(aspec)
+    q2 = _alphas_points(aspec, np.random.default_rng(6), 200_003)
+    dq = torch.from_numpy(q2).cuda()
+    out, out_q = torch.empty_like(dq), torch.empty_like(dq)
+    B.alphas_q2(ha, dq, out)
+    q = np.sqrt(np.where(q2 > 0, q2, np.nan))
+    B.alphas_q(ha, torch.from_numpy(q).cuda(), out_q)
+    torch.cuda.synchronize()
+    oa = oracle.OracleAlphas.from_spec(aspec)
+    st = check_parity(out.cpu().numpy(), oa.q2(q2), what="alphas 300 nodes (k_alphas)")
+    assert st["n_clause"] == 0
+    check_parity(out_q.cpu().numpy(), oa.q2(q * q), what="alphas_q 300 nodes (k_alphas)")
+    B.alphas_grid_free(ha)
+    # the largest list the library takes, and one node too many
+    big = W.make_alphas_grid(nq_per_sub=(32, 64, 160, 256))
+    hb = B.load_alphas_spec(big)
+    q2 = _alphas_points(big, np.random.default_rng(7), 50_001)
+    dq = torch.from_numpy(q2).cuda()
+    out = torch.empty_like(dq)
+    B.alphas_q2(hb, dq, out)
+    torch.cuda.synchronize()
+    check_parity(out.cpu().numpy(), oracle.OracleAlphas.from_spec(big).q2(q2), what="alphas 512 nodes")
+    B.alphas_grid_free(hb)
+    with pytest.raises(B.PdfbError):
+        B.load_alphas_spec(W.make_alphas_grid(nq_per_sub=(32, 64, 160, 257)))
+
+
+@pytest.mark.parametrize("nodes", [(6, 12, 30, 52), (20, 40, 100, 140)])
+def test_alphas_q2_host_entry(torch_cuda, nodes):
+    """alphas_q2_host (host buffers, chunked pipeline): bit-identical to alphas_q2 on the same
+    points, more than one pipeline chunk with a ragged tail, and within tolerance of the oracle."""
+    torch = torch_cuda
+    aspec = W.make_alphas_grid(nq_per_sub=nodes)
+    ha = B.load_alphas_spec(aspec)
+    n = 9_000_011
+    rng = np.random.default_rng(8)
+    q2 = np.exp(rng.uniform(np.log(0.5), np.log(4e10), n))
+    q2[:5] = [0.0, -1.0, np.nan, aspec.q_knots[0] ** 2, aspec.q_knots[-1] ** 2]
+    out_h = np.empty(n)
+    B.alphas_q2_host(ha, q2, out_h)
+    dq = torch.from_numpy(q2).cuda()
+    out_d = torch.empty_like(dq)
+    B.alphas_q2(ha, dq, out_d)
+    torch.cuda.synchronize()
+    assert np.array_equal(out_h, out_d.cpu().numpy(), equal_nan=True)
+    idx = np.concatenate([np.arange(64), rng.integers(0, n, 200_000), np.arange(n - 64, n)])
+    check_parity(out_h[idx], oracle.OracleAlphas.from_spec(aspec).q2(q2[idx]), what=f"alphas_q2_host {sum(nodes)} nodes")
+    B.alphas_q2_host(ha, q2[:0], out_h[:0])      # empty batch
+    B.alphas_grid_free(ha)
+
+
+def test_forced_fallback_kernel_on_the_nnpdf_grid(torch_cuda, grid2, ograph2, monkeypatch):
+    """PDFB_FORCE_FALLBACK=1 at load: k_xfxq2_v0 (one thread per point, read-only cache) on the
+    NNPDF-shaped grid -- the config-4 mix, the knot/threshold scan, PID subsets, the Q entry."""
+    torch = torch_cuda
+    monkeypatch.setenv("PDFB_FORCE_FALLBACK", "1")
+    h = B.load_pdf_spec(grid2)
+    monkeypatch.delenv("PDFB_FORCE_FALLBACK")
+    assert not B.pdf_grid_uses_smem_path(h)
+    pids = list(W.PIDS_11)
+    x, q2 = W.queries_extrapolation_mix(grid2, 150_007)
+    xs, qs = W.scan_points(grid2, per_cell=2)
+    x, q2 = np.concatenate([x, xs]), np.concatenate([q2, qs])
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    for req in (pids, [21], [0, -5, 3, 3]):
+        out = torch.empty((len(req), len(x)), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h, req, dx, dq, out)
+        torch.cuda.synchronize()
+        ref, sc = ograph2.xfxq2(req, x, q2, with_scale=True)
+        st = check_parity(out.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what=f"forced k_xfxq2_v0 {req}")
+        print("fallback", req, st)
+    out_q = torch.empty((len(pids), len(x)), dtype=torch.float64, device="cuda")
+    out_2 = torch.empty_like(out_q)
+    q = np.sqrt(q2)
+    B.pdf_xfxq(h, pids, dx, torch.from_numpy(q).cuda(), out_q)
+    B.pdf_xfxq2(h, pids, dx, torch.from_numpy(q * q).cuda(), out_2)
+    torch.cuda.synchronize()
+    assert torch.equal(out_q, out_2)
+    # knots reproduced bit for bit on this path too
+    X, Q = np.meshgrid(grid2.x_knots, grid2.sub_q(1) ** 2, indexing="ij")
+    out = torch.empty((len(pids), X.size), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h, pids, torch.from_numpy(X.ravel().copy()).cuda(), torch.from_numpy(Q.ravel().copy()).cuda(), out)
+    assert np.array_equal(out.cpu().numpy(), grid2.sub_values(1).transpose(2, 0, 1).reshape(len(pids), -1))
+    B.pdf_grid_free(h)
+
+
+@pytest.mark.parametrize("force_fallback", [False, True])
+def test_rule_C_small_y0_branch(torch_cuda, monkeypatch, force_fallback):
+    """Q^2 < q_min with |y0| on either side of 1e-5 (reading Q9: gamma = 1 below it): a grid whose
+    q_min row crosses 1e-5 along x, so both branches occur in one batch, on both kernels."""
+    torch = torch_cuda
+    from test_oracle_pins import make_spec
+    xk = np.geomspace(1e-5, 1.0, 24)
+    qk = np.geomspace(1.5, 300.0, 9)
+
+    def fn(s, x, q2, pid):
+        amp = 3e-4 if pid == 21 else -2e-4
+        return amp * x ** 0.4 * (1.0 - x) ** 2 * (q2 / qk[0] ** 2) ** (0.25 if pid == 21 else -0.6)
+
+    spec = make_spec(xk, [qk], [1, 21], fn)
+    if force_fallback:
+        monkeypatch.setenv("PDFB_FORCE_FALLBACK", "1")
+    h = B.load_pdf_spec(spec)
+    monkeypatch.delenv("PDFB_FORCE_FALLBACK", raising=False)
+    assert bool(B.pdf_grid_uses_smem_path(h)) != force_fallback
+    rng = np.random.default_rng(3)
+    n = 60_001
+    x = np.exp(rng.uniform(np.log(1e-7), 0.0, n))
+    q2 = spec.q2_min * np.exp(rng.uniform(np.log(1e-3), 0.0, n)) * (1 - 1e-12)
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    y0 = og.xfxq2([1, 21], np.clip(x, xk[0], 1.0), np.full(n, spec.q2_min))
+    frac_small = (np.abs(y0) < 1e-5).mean()
+    assert 0.2 < frac_small < 0.8, frac_small       # both branches are well populated
+    out = torch.empty((2, n), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h, [1, 21], torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), out)
+    torch.cuda.synchronize()
+    ref, sc = og.xfxq2([1, 21], x, q2, with_scale=True)
+    st = check_parity(out.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what=f"rule C small y0, fallback={force_fallback}")
+    print(st)
+    B.pdf_grid_free(h)
