@@ -2,6 +2,8 @@
 // extrapolation (reading O6; "log-cubic interpolation with constant extrapolation
 // from the (alpha_s(Q), Q) nodes ... improved treatment of the sub-grids mechanism").
 // The whole node table (knots, values, interval records: 80 B per node) lives in shared memory.
+#include <atomic>
+
 #include "pdfb_internal.cuh"
 
 #define ALPHAS_SMEM_MAX_KNOTS 512
@@ -114,14 +116,17 @@ int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, doub
 {
     if (n == 0) return PDFB_OK;
     if (a->d.fast_ok) {
-        static int attr_dev = -1;
-        if (attr_dev != a->device) {
+        // the attribute is per function and device; setting it twice is harmless, so a relaxed
+        // per-device bit is enough for concurrent callers
+        static std::atomic<unsigned long long> attr_done{0};
+        const unsigned long long bit = 1ULL << (a->device & 63);
+        if (!(attr_done.load(std::memory_order_acquire) & bit)) {
             PDFB_CUDA(cudaFuncSetAttribute(k_alphas_fast<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
             PDFB_CUDA(cudaFuncSetAttribute(k_alphas_fast<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 110 * 1024));
-            attr_dev = a->device;
+            attr_done.fetch_or(bit, std::memory_order_release);
         }
         long long blocks = (n + NT_ALPHAS - 1) / NT_ALPHAS;
-        if (blocks > 148 * CTAS_ALPHAS) blocks = 148 * CTAS_ALPHAS;
+        if (blocks > (long long)a->sms * CTAS_ALPHAS) blocks = (long long)a->sms * CTAS_ALPHAS;
         if (q_is_q) k_alphas_fast<true><<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
         else k_alphas_fast<false><<<(unsigned)blocks, NT_ALPHAS, a->d.fast_bytes, st>>>(a->d, n, q2, out);
         pdfb_count_launch(1);
@@ -130,7 +135,7 @@ int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, doub
     }
     size_t smem = (size_t)a->d.K * (sizeof(IntervalRec) + 16);
     long long blocks = (n + 255) / 256;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > (long long)a->sms * 8) blocks = (long long)a->sms * 8;
     k_alphas<<<(unsigned)blocks, 256, smem, st>>>(a->d, n, q2, out, q_is_q);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());

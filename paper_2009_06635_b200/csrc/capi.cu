@@ -82,14 +82,18 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
         for (long long e = 0; e < tot; e++) if (!std::isfinite(values[e])) return PDFB_EINVAL;
     }
 
+    if (!(x_knots[0] >= 1e-300) || !(q_knots[0] * q_knots[0] >= 1e-300)) return PDFB_EKNOTS;  // subnormal coordinates
+
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return PDFB_ECUDA;
-    PDFB_CUDA(cudaSetDevice(device));
+    DeviceGuard guard(device);  // the caller's current device is put back on return
+    if (!guard.ok) return PDFB_ECUDA;
 
     pdfb_grid *g = new (std::nothrow) pdfb_grid();
     if (!g) return PDFB_EINVAL;
     memset(g, 0, sizeof(*g));
     g->device = device;
+    if (cudaDeviceGetAttribute(&g->sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { delete g; return PDFB_ECUDA; }
     GridDev &d = g->d;
     d.n_sub = n_sub; d.nx = nx; d.n_pid = n_pid; d.nq_tot = nq_tot; d.n_members = n_members;
     d.kpad = (n_pid + 1) & ~1;  // even number of doubles per knot: 16-byte aligned knots
@@ -100,7 +104,6 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     std::vector<double> h_q2(nq_tot + 1), h_z(nx + nq_tot + 1);
     for (int j = 0; j < nq_tot; j++) h_q2[j] = q_knots[j] * q_knots[j];
     h_q2[nq_tot] = 1.01 * h_q2[0];  // rule C's second probe scale rides along
-    if (!(x_knots[0] >= 1e-300) || !(h_q2[0] >= 1e-300)) return PDFB_EKNOTS;
     long long knots = 0;
     for (int s = 0; s < n_sub; s++) {
         d.q_off[s] = q_offsets[s];
@@ -153,8 +156,12 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     g->blob = blob; g->blob_bytes = total;
 
     int rc = PDFB_OK;
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        if (e0) cudaEventDestroy(e0);
+        cudaFree(blob); delete g;
+        return PDFB_ECUDA;
+    }
     do {
         if (cudaMemcpy(blob + o_xk, x_knots, sizeof(double) * nx, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(blob + o_q2k, h_q2.data(), sizeof(double) * (nq_tot + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
@@ -274,6 +281,8 @@ static int members_impl(const pdfb_grid *g, int member0, int n_mem, int n_req, c
     int rc = resolve_cols(g, n_req, pids, cols);
     if (rc) return rc;
     if (n_mem == 0) return PDFB_OK;
+    DeviceGuard guard(g->device);
+    if (!guard.ok) return PDFB_ECUDA;
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream, q_is_q, member0, n_mem);
 }
 
@@ -297,6 +306,8 @@ extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long lo
     int cols[PDFB_MAX_PIDS];
     int rc = resolve_cols(g, n_req, pids, cols);
     if (rc) return rc;
+    DeviceGuard guard(g->device);
+    if (!guard.ok) return PDFB_ECUDA;
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream);
 }
 
@@ -308,6 +319,8 @@ extern "C" int pdf_xfxq(const pdfb_grid *g, int n_req, const int *pids, long lon
     int cols[PDFB_MAX_PIDS];
     int rc = resolve_cols(g, n_req, pids, cols);
     if (rc) return rc;
+    DeviceGuard guard(g->device);
+    if (!guard.ok) return PDFB_ECUDA;
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q, out, n, (cudaStream_t)cuda_stream, 1);
 }
 
@@ -317,7 +330,8 @@ extern "C" int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points)
 {
     if (!g || !n_invalid_points) return PDFB_EINVAL;
     unsigned long long c = 0;
-    PDFB_CUDA(cudaSetDevice(g->device));
+    DeviceGuard guard(g->device);
+    if (!guard.ok) return PDFB_ECUDA;
     PDFB_CUDA(cudaDeviceSynchronize());
     PDFB_CUDA(cudaMemcpy(&c, g->d.n_invalid, sizeof(c), cudaMemcpyDeviceToHost));
     *n_invalid_points = (long long)c;
@@ -327,12 +341,10 @@ extern "C" int pdf_grid_status(const pdfb_grid *g, long long *n_invalid_points)
 extern "C" void pdf_grid_free(pdfb_grid *g)
 {
     if (!g) return;
-    cudaSetDevice(g->device);
+    DeviceGuard guard(g->device);
     cudaDeviceSynchronize();
-    for (int i = 0; i < 3; i++) {
+    for (int i = 0; i < 3; i++)
         if (g->streams[i]) cudaStreamDestroy(g->streams[i]);
-        if (g->ev_done[i]) cudaEventDestroy(g->ev_done[i]);
-    }
     if (g->stage) cudaFree(g->stage);
     if (g->blob) cudaFree(g->blob);
     delete g;

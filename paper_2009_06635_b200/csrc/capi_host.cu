@@ -30,18 +30,21 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
     if (n_sub > PDFB_MAX_SUBGRIDS) return PDFB_ELIMIT;
     for (int s = 0; s < n_sub; s++) if (off[s + 1] - off[s] < 2) return PDFB_EKNOTS;
 
+    if (!(q_knots[0] * q_knots[0] >= 1e-300)) return PDFB_EKNOTS;  // subnormal scale
+
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return PDFB_ECUDA;
-    PDFB_CUDA(cudaSetDevice(device));
+    DeviceGuard guard(device);
+    if (!guard.ok) return PDFB_ECUDA;
     pdfb_alphas *a = new (std::nothrow) pdfb_alphas();
     if (!a) return PDFB_EINVAL;
     memset(a, 0, sizeof(*a));
     a->device = device;
+    if (cudaDeviceGetAttribute(&a->sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { delete a; return PDFB_ECUDA; }
     AlphasDev &d = a->d;
     d.K = n_knots; d.n_sub = n_sub;
     std::vector<double> h_q2(n_knots), h_z(n_knots);
     for (int k = 0; k < n_knots; k++) h_q2[k] = q_knots[k] * q_knots[k];
-    if (!(h_q2[0] >= 1e-300)) return PDFB_EKNOTS;
     for (int s = 0; s <= n_sub; s++) d.off[s] = off[s];
     for (int s = 0; s < n_sub; s++) d.q2_lo[s] = h_q2[off[s]];
     d.q2_min = h_q2[0]; d.q2_max = h_q2[n_knots - 1];
@@ -89,6 +92,8 @@ extern "C" int alphas_q2(const pdfb_alphas *a, long long n, const double *q2, do
 {
     if (!a || n < 0) return PDFB_EINVAL;
     if (n > 0 && (!q2 || !out)) return PDFB_EINVAL;
+    DeviceGuard guard(a->device);
+    if (!guard.ok) return PDFB_ECUDA;
     return pdfb_launch_alphas(a, n, q2, out, (cudaStream_t)cuda_stream);
 }
 
@@ -96,13 +101,15 @@ extern "C" int alphas_q(const pdfb_alphas *a, long long n, const double *q, doub
 {
     if (!a || n < 0) return PDFB_EINVAL;
     if (n > 0 && (!q || !out)) return PDFB_EINVAL;
+    DeviceGuard guard(a->device);
+    if (!guard.ok) return PDFB_ECUDA;
     return pdfb_launch_alphas(a, n, q, out, (cudaStream_t)cuda_stream, 1);
 }
 
 extern "C" void alphas_grid_free(pdfb_alphas *a)
 {
     if (!a) return;
-    cudaSetDevice(a->device);
+    DeviceGuard guard(a->device);
     cudaDeviceSynchronize();
     for (int i = 0; i < 2; i++) if (a->streams[i]) cudaStreamDestroy(a->streams[i]);
     if (a->stage) cudaFree(a->stage);
@@ -127,7 +134,8 @@ extern "C" int pdf_xfxq2_host(pdfb_grid *g, int n_req, const int *pids, long lon
         for (int k = 0; k < g->d.n_pid; k++) if (g->pids[k] == pid) cols[r] = k;
         if (cols[r] < 0) return PDFB_EPID;
     }
-    PDFB_CUDA(cudaSetDevice(g->device));
+    DeviceGuard guard(g->device);
+    if (!guard.ok) return PDFB_ECUDA;
     const int NS = 3;
     const long long chunk = n < HOST_CHUNK ? n : HOST_CHUNK;
     const size_t per_stage = sizeof(double) * chunk * (2 + (size_t)n_req);
@@ -152,8 +160,10 @@ extern "C" int pdf_xfxq2_host(pdfb_grid *g, int n_req, const int *pids, long lon
             cudaMemcpyAsync(dq, q2 + a, sizeof(double) * m, cudaMemcpyHostToDevice, st) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         rc = pdfb_launch_xfxq2(g, n_req, cols, m, dx, dq, dout, chunk, st);
         if (rc) break;
-        if (cudaMemcpy2DAsync(out + a, sizeof(double) * n, dout, sizeof(double) * chunk, sizeof(double) * m, n_req,
-                              cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = PDFB_ECUDA;
+        // one copy per flavour row (a 2-D copy would cap the pitch 8 n at cudaDevAttrMaxPitch: n < 2^28)
+        for (int r = 0; r < n_req && !rc; r++)
+            if (cudaMemcpyAsync(out + (size_t)r * n + a, dout + (size_t)r * chunk, sizeof(double) * m, cudaMemcpyDeviceToHost, st) != cudaSuccess)
+                rc = PDFB_ECUDA;
     }
     for (int i = 0; i < NS; i++) if (cudaStreamSynchronize(g->streams[i]) != cudaSuccess) rc = rc ? rc : PDFB_ECUDA;
     return rc;
@@ -164,7 +174,8 @@ extern "C" int alphas_q2_host(pdfb_alphas *a, long long n, const double *q2, dou
     if (!a || n < 0) return PDFB_EINVAL;
     if (n == 0) return PDFB_OK;
     if (!q2 || !out) return PDFB_EINVAL;
-    PDFB_CUDA(cudaSetDevice(a->device));
+    DeviceGuard guard(a->device);
+    if (!guard.ok) return PDFB_ECUDA;
     const int NS = 2;
     const long long chunk = n < HOST_CHUNK ? n : HOST_CHUNK;
     const size_t per_stage = sizeof(double) * chunk * 2;

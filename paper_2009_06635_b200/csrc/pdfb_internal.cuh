@@ -39,8 +39,20 @@ __host__ __device__ __forceinline__ void weights4(const IntervalRec &r, double t
 
 // ---------------------------------------------------------------------------------------------
 // ln of a positive, finite, normal double.  Classic argument reduction m in [sqrt(1/2), sqrt(2)),
-// s = f/(2+f), odd series in s (coefficients of the fdlibm/FreeBSD e_log.c minimax fit, < 1 ulp);
-// coefficients live in constant memory so that they are operands, not moves.
+// s = f/(2+f), odd series in s, < 1 ulp; coefficients live in constant memory so that they are
+// operands, not moves.  The reduction constant, the split of ln 2 and the minimax coefficients
+// Lg1..Lg7 below are those of fdlibm's e_log.c, whose notice is reproduced as its licence asks:
+//
+//   ====================================================
+//   Copyright (C) 1993 by Sun Microsystems, Inc. All rights reserved.
+//
+//   Developed at SunSoft, a Sun Microsystems, Inc. business.
+//   Permission to use, copy, modify, and distribute this
+//   software is freely granted, provided that this notice
+//   is preserved.
+//   ====================================================
+//
+// (the division of that routine is replaced here by a reciprocal seed + Newton steps + residual).
 static __constant__ double c_ln[10] = {
     6.93147180369123816490e-01,  // ln2_hi
     1.90821492927058770002e-10,  // ln2_lo
@@ -109,7 +121,7 @@ struct GridDev {
     const IntervalRec *qrec;           // [nq_tot]; entry q_off[s]+j = interval j of sub-grid s
     const double *val;                 // [member][s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
     unsigned long long *n_invalid;     // sticky counter
-    uint32_t *slow_ws;                 // smem path: per-SM, per-warp, per-class lists of out-of-grid points
+    uint32_t *slow_ws;                 // smem path: per SM and warp, PDFB_SLOW_CLASSES lists of out-of-grid point indices
     // ---- shared-memory path (xfxq2_smem.cu): flavour-group slices + a small aux block
     int smem_ok;                       // bit 0: the 4-column slices fit shared memory; bit 1: the 2-column ones
                                        // (0 if nx < 4 or a sub-grid has < 4 Q knots: read-only-cache kernel)
@@ -131,8 +143,12 @@ struct GridDev {
 #define PDFB_LUT_BINS 512
 #endif
 #define PDFB_SLOW_CLASSES 5   // x < x_min | Q^2 > max | Q^2 < min | the two corners
-#define PDFB_WS_SLOTS 256     // >= %nsmid: one scratch slot per SM
-#define PDFB_WS_BYTES (PDFB_WS_SLOTS * 32 * PDFB_SLOW_CLASSES * 32 * 4)  // up to 32 warps per CTA
+#define PDFB_WS_SLOTS 160     // >= %nsmid (148 on B200; checked at load): one scratch slot per SM
+#ifndef PDFB_SLOW_TRIGGER
+#define PDFB_SLOW_TRIGGER 192  // a list this long asks every warp of the CTA to evaluate its full batches
+#endif
+#define PDFB_SLOW_LCAP 256     // entries per warp and class list; 8-bit counters: TRIGGER - 1 + 32 + 31 <= 255
+#define PDFB_WS_BYTES ((size_t)PDFB_WS_SLOTS * 16 * PDFB_SLOW_CLASSES * PDFB_SLOW_LCAP * 4)  // 16 warps per CTA
 // Shared-memory image of the smem path: [pre | slice | post].
 //   pre  = lutx, lutq, raw x knots, raw Q^2 knots, then xrec;   post = qrec, then zero padding.
 // xrec/qrec = 128-byte lines holding 4 copies of the 32-byte IntervalRec32 of an interval (qrec is
@@ -167,8 +183,22 @@ struct AlphasDev {
     double lut_v0, lut_inv_h;
 };
 
+// Makes the handle's device current for the duration of a call and puts the caller's device back.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int device)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; ok = false; return; }
+        if (prev != device) { if (cudaSetDevice(device) != cudaSuccess) ok = false; }
+        else prev = -1;  // nothing to restore
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 struct pdfb_grid {
     int device;
+    int sms;                  // multiprocessors of `device`
     GridDev d;
     int pids[PDFB_MAX_PIDS];
     void *blob;               // one device allocation holding all tables
@@ -177,12 +207,12 @@ struct pdfb_grid {
     void *stage;
     size_t stage_bytes;
     cudaStream_t streams[3];
-    cudaEvent_t ev_done[3];
     double setup_ms;
 };
 
 struct pdfb_alphas {
     int device;
+    int sms;
     AlphasDev d;
     void *blob;
     void *stage;

@@ -23,347 +23,10 @@
 //   * the x weights are rotated the same way (selects on the ALU pipe), so no data is moved back.
 // Knot location uses a uniform-in-log lookup table corrected by comparisons on the raw knots
 // (the result is defined by the comparisons, reading Q5).
+#include <atomic>
 #include <cstdlib>
 
-#include "pdfb_internal.cuh"
-
-struct PassList {
-    int n;
-    int group[PDFB_MAX_PIDS];
-    int row[PDFB_MAX_PIDS][4];  // output row of each of the group's 4 columns, -1 = not requested
-};
-
-#ifndef NT_SMEM
-#define NT_SMEM 512   // threads per CTA (one CTA per SM: the slice fills shared memory)
-#endif
-#ifndef PPT_SMEM
-#define PPT_SMEM 1    // points per thread and tile
-#endif
-
-__device__ __forceinline__ double2 lds128(uint32_t addr)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
-}
-
-// The continuation rules run on a few percent of the points at most but carry the fp64 log / exp /
-// pow bodies: they are kept OUT of line (one copy each) so that the kernel stays within the
-// instruction cache when warps alternate between the fast path and the out-of-grid lists
-// (inlined they made the kernel 112 KB and a 30 % out-of-grid mix 3x slower than its parts).
-__device__ __noinline__ double cont_e(double r, double yL, double yH)  // reading O4
-{
-    if (yL > 1e-3 && yH > 1e-3) {
-        double lL = log(yL);
-        return exp(fma(r, log(yH) - lL, lL));
-    }
-    return fma(r, yH - yL, yL);
-}
-
-// the coordinate logarithm of the out-of-grid path: pdfb_ln, one copy (code size, see cont_e)
-__device__ __noinline__ double ln_slow(double a) { return pdfb_ln(a); }
-
-// rule C (reading O5): y0 * rho^(gamma*rho + 1 - rho), gamma from the probe at 1.01 q_min;
-// |y0| < 1e-5: gamma = 1, i.e. y0 * rho (reading Q9)
-__device__ __noinline__ double rule_c(double y0, double y1, double rho)
-{
-    double gamma = 1.0;
-    if (fabs(y0) >= 1e-5) gamma = fmax(-2.5, (y1 - y0) / y0 / 0.01);
-    return y0 * pow(rho, fma(gamma, rho, 1.0 - rho));
-}
-
-// The four 1-D weights of knots m-1..m+2 from the 32-byte interval record.  aLm == 0 marks the
-// first interval of the knot array (knot m-1 does not exist, weight exactly 0), aHp == 0 the last.
-__device__ __forceinline__ void weights_rec32(const IntervalRec32 &r, double t, double w[4])
-{
-    // exact zero tests on the high words (the records hold +0.0 there), off the FP64 pipe
-    const bool first = (__double2hiint(r.aLm) << 1) == 0, last = (__double2hiint(r.aHp) << 1) == 0;
-    double t2 = t * t, t3 = t2 * t;
-    double h01 = 3.0 * t2 - 2.0 * t3;
-    double h00 = 1.0 - h01;
-    double h11 = t3 - t2;
-    double h10 = h11 - t2 + t;
-    double aL1 = first ? 1.0 : 0.5, aH0 = last ? -1.0 : -0.5;
-    double aL0 = -(r.aLm + aL1), aH1 = -(aH0 + r.aHp);
-    w[0] = h10 * r.aLm;
-    w[1] = fma(h11, aH0, fma(h10, aL0, h00));
-    w[2] = fma(h11, aH1, fma(h10, aL1, h01));
-    w[3] = h11 * r.aHp;
-}
-
-// o[k] = w[(k + r) & 3]
-__device__ __forceinline__ void rot4(const double w[4], int r, double o[4])
-{
-    double a[4];
-#pragma unroll
-    for (int k = 0; k < 4; k++) a[k] = (r & 1) ? w[(k + 1) & 3] : w[k];
-#pragma unroll
-    for (int k = 0; k < 4; k++) o[k] = (r & 2) ? a[(k + 2) & 3] : a[k];
-}
-
-// The x side of a point's stencil.  The 128-byte run of knots node0..node0+3 (node0 = i-1, 4
-// columns each) holds chunk c = 2*(knot - node0) + (column pair).  Lane l reads, at step s,
-//   c(s) = ((s + rot) & 7) ^ (l & 1),   rot = ((l & 6) - 2*node0) & 7   (even),
-// which puts the 8 lanes of a quarter-warp on 8 distinct bank groups at every step.  Steps 2k and
-// 2k+1 both belong to knot (k + rot/2) & 3, so one rotated weight W[k] serves both; even steps
-// deliver column pair (l & 1), odd steps the other pair (swapped back before the store).
-struct Win { uint32_t a[8]; double W[4]; };
-
-// row0 = shared address of stencil row 0 (table row gi-1); wu = x weights of knots node0..node0+3
-__device__ __forceinline__ void make_win(Win &u, uint32_t row0, int node0, const double wu[4], int lane8)
-{
-    const int rot2 = ((lane8 >> 1) - node0) & 3;
-    const uint32_t base = row0 + (uint32_t)(node0 * 32) + ((uint32_t)(lane8 & 1) << 4);
-#pragma unroll
-    for (int k = 0; k < 4; k++) {
-        u.a[2 * k] = base + ((uint32_t)((k + rot2) & 3) << 5);
-        u.a[2 * k + 1] = u.a[2 * k] ^ 16u;
-    }
-    rot4(wu, rot2, u.W);
-}
-
-// sum_b vw[b] * sum_k W[k] * V[window row b][window knot][cols] -> E = column pair (lane & 1), O = the other
-__device__ __forceinline__ void gather4(const Win &u, const double vw[4], uint32_t rb1, uint32_t rb2, uint32_t rb3,
-                                        double2 &yE, double2 &yO)
-{
-    yE = make_double2(0.0, 0.0); yO = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int b = 0; b < 4; b++) {
-        const uint32_t ro = (b == 0) ? 0u : (b == 1) ? rb1 : (b == 2) ? rb2 : rb3;
-        double2 c[8];
-#pragma unroll
-        for (int s = 0; s < 8; s++) c[s] = lds128(u.a[s] + ro);
-        double2 E, O;
-        E.x = u.W[0] * c[0].x; E.y = u.W[0] * c[0].y;
-        O.x = u.W[0] * c[1].x; O.y = u.W[0] * c[1].y;
-#pragma unroll
-        for (int k = 1; k < 4; k++) {
-            E.x = fma(u.W[k], c[2 * k].x, E.x); E.y = fma(u.W[k], c[2 * k].y, E.y);
-            O.x = fma(u.W[k], c[2 * k + 1].x, O.x); O.y = fma(u.W[k], c[2 * k + 1].y, O.y);
-        }
-        yE.x = fma(vw[b], E.x, yE.x); yE.y = fma(vw[b], E.y, yE.y);
-        yO.x = fma(vw[b], O.x, yO.x); yO.y = fma(vw[b], O.y, yO.y);
-    }
-}
-
-// ---- 2-column slices (16 B per knot).  A 4-knot run is 64 bytes = 4 bank groups; the row length is
-// 64 (mod 128) bytes, so the same run one row further down covers the other 4.  A ROW PAIR is read as
-// one virtual run of 8 chunks: chunk v < 4 = (upper row, knot v), v >= 4 = (lower row, knot v - 4),
-// bank group (g0 + v) & 7.  Lane l reads v(s) = (s + l - g0) & 7 at step s: the 8 lanes of a
-// quarter-warp are on 8 distinct bank groups whatever their cells.  16 conflict-free LDS.128 per
-// point, each delivering both columns of one knot (no column-pair parity here).
-__device__ __forceinline__ void stencil2(uint32_t row0, uint32_t RB, int node0, const double wu[4], const double vw[4],
-                                         int lane8, double out[2])
-{
-    const uint32_t base = row0 + (uint32_t)(node0 * 16);
-    const int rho = (lane8 - (int)(base >> 4)) & 7;  // g0 = bank group of the run's first chunk
-    double Wr[4];
-    rot4(wu, rho & 3, Wr);  // Wr[j] = weight of the knot read at steps s = j, j + 4
-    uint32_t a[8];
-    bool low[8];            // step s reads the lower row of the pair
-#pragma unroll
-    for (int s = 0; s < 8; s++) {
-        const int v = (s + rho) & 7;
-        low[s] = v >> 2;
-        a[s] = base + (uint32_t)((v & 3) << 4) + (low[s] ? RB : 0u);
-    }
-    double y0 = 0.0, y1 = 0.0;
-#pragma unroll
-    for (int p = 0; p < 2; p++) {  // row pairs (0,1) and (2,3)
-        double2 c[8];
-#pragma unroll
-        for (int s = 0; s < 8; s++) c[s] = lds128(a[s] + (p ? 2u * RB : 0u));
-#pragma unroll
-        for (int s = 0; s < 8; s++) {
-            const double w = Wr[s & 3] * (low[s] ? vw[2 * p + 1] : vw[2 * p]);
-            y0 = fma(w, c[s].x, y0); y1 = fma(w, c[s].y, y1);
-        }
-    }
-    out[0] = y0; out[1] = y1;
-}
-
-// One stencil evaluation on a W-column slice: first stencil row `row` (table row gi-1), first knot
-// node0 (= i-1); values come back in column order.
-template <int W>
-__device__ __forceinline__ void eval_stencil(uint32_t tab, uint32_t RB, uint32_t RB2, uint32_t RB3, int row, int node0,
-                                             const double wu[4], const double vw[4], int lane8, double out[W])
-{
-    const uint32_t row0 = tab + (uint32_t)(row * (int)RB);
-    if (W == 4) {
-        Win w;
-        make_win(w, row0, node0, wu, lane8);
-        double2 E, O;
-        gather4(w, vw, RB, RB2, RB3, E, O);
-        const bool odd = lane8 & 1;  // E / O are the column pairs (lane & 1) / the other: back to column order
-        out[0] = odd ? O.x : E.x; out[1] = odd ? O.y : E.y; out[W - 2] = odd ? E.x : O.x; out[W - 1] = odd ? E.y : O.y;
-    } else {
-        stencil2(row0, RB, node0, wu, vw, lane8, out);
-    }
-}
-
-struct SmemViews {
-    uint32_t tab, row_bytes, xrec, qrec;  // shared-space byte addresses
-    const double *xk, *q2k;
-    const unsigned short *lutx, *lutq;
-};
-
-// shared memory = [pre | slice | post] (pdfb_internal.cuh); the slice has W columns per knot
-template <int W>
-__device__ __forceinline__ SmemViews make_views(const GridDev &g, unsigned char *smem)
-{
-    SmemViews sv;
-    const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(smem);
-    sv.tab = s0 + (uint32_t)g.pre_bytes;
-    sv.row_bytes = (W == 4) ? (uint32_t)g.nx4 * 32u : (uint32_t)g.nx2 * 16u;
-    sv.xrec = s0 + (uint32_t)g.a_xrec;
-    sv.qrec = sv.tab + (uint32_t)((W == 4 ? g.slice_bytes : g.slice2_bytes) + g.a_qrec);
-    sv.xk = reinterpret_cast<const double *>(smem + g.a_xk);
-    sv.q2k = reinterpret_cast<const double *>(smem + g.a_q2k);
-    sv.lutx = reinterpret_cast<const unsigned short *>(smem + g.a_lutx);
-    sv.lutq = reinterpret_cast<const unsigned short *>(smem + g.a_lutq);
-    return sv;
-}
-
-// 32-byte interval record from its 128-byte line of 4 copies: lanes 2k and 2k+1 of a
-// quarter-warp use copy k and read its two 16-byte halves in opposite order, so the 8 lanes
-// touch 8 distinct bank groups at both steps whatever records they want.
-__device__ __forceinline__ IntervalRec32 load_rec4(uint32_t line, int lane8)
-{
-    const uint32_t copy = line + (uint32_t)((lane8 >> 1) << 5);
-    const uint32_t h = (uint32_t)(lane8 & 1) << 4;
-    const double2 A = lds128(copy + h), B = lds128(copy + (h ^ 16u));
-    IntervalRec32 r;
-    r.z0 = h ? B.x : A.x; r.inv_dz = h ? B.y : A.y;
-    r.aLm = h ? A.x : B.x; r.aHp = h ? A.y : B.y;
-    return r;
-}
-
-// Interval search: LUT guess (pdfb_internal.cuh) + at most one comparison on the raw knots; bins
-// holding several distinct knots take the comparison loop.  Returns the last m <= kmax with
-// knots[m] <= val (the result is defined by the comparisons, reading Q5).
-__device__ __forceinline__ int locate(const unsigned short *lut, const double *knots, int kmax, double val,
-                                      double z, double z0, double inv_h)
-{
-    const int b = min(max((int)((z - z0) * inv_h), 0), PDFB_LUT_BINS - 1);
-    const int e = lut[b], d = (e >> 1) & 3;
-    int m = e >> 3;
-    if (d) { if (knots[m + d] <= val) m += d; }
-    if (e & 1)
-        while (m < kmax && knots[m + 1] <= val) ++m;
-    return m;
-}
-
-__device__ __forceinline__ int locate_x(const GridDev &g, const SmemViews &sv, double xv, double u)
-{
-    return locate(sv.lutx, sv.xk, g.nx - 2, xv, u, g.lutx_u0, g.lutx_inv_h);
-}
-
-// Interval of Q^2 as an index into the CONCATENATED knot list.  A threshold is stored twice (last
-// knot of the lower sub-grid, first of the upper), so a point on it lands on the upper copy
-// (reading Q2) and the lower copy never starts an interval; only Q^2 = q2_max needs the clamp.
-// Interval records and table rows use the same index.
-__device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, double qv, double v)
-{
-    return min(locate(sv.lutq, sv.q2k, g.nq_tot - 1, qv, v, g.lutq_v0, g.lutq_inv_h), g.nq_tot - 2);
-}
-
-template <int W> struct YW { double v[W]; };  // one point's W columns, in column order
-
-// one stencil evaluation of the out-of-grid path, out of line (see cont_e)
-template <int W>
-__device__ __noinline__ YW<W> probe(uint32_t tab, uint32_t RB, int row, int node0, const double *wu, const double *vw, int lane8)
-{
-    const double wu4[4] = {wu[0], wu[1], wu[2], wu[3]}, vw4[4] = {vw[0], vw[1], vw[2], vw[3]};
-    YW<W> r;
-    eval_stencil<W>(tab, RB, 2u * RB, 3u * RB, row, node0, wu4, vw4, lane8, r.v);
-    return r;
-}
-
-// points outside the grid (readings O4/O5): up to 2 x-sets times 2 row sets
-template <int W>
-__device__ __noinline__ YW<W> slow_point(const GridDev *gp, unsigned char *smem, double xv, double qv, int lane8)
-{
-    const GridDev &g = *gp;
-    const SmemViews sv = make_views<W>(g, smem);
-    const uint32_t RB = sv.row_bytes;
-    const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
-    // ---- x: one weight set in range, else the two one-hot sets of knots 0 and 1 (rule A)
-    double wu1[4] = {1.0, 0.0, 0.0, 0.0}, wu2[4] = {0.0, 1.0, 0.0, 0.0};  // knots 0..3
-    int node0 = 0;
-    double rA = 0.0;
-    if (!low_x) {
-        const double u = ln_slow(xv);
-        const int i = locate_x(g, sv, xv, u);
-        const IntervalRec32 r = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
-        weights_rec32(r, (u - r.z0) * r.inv_dz, wu1);
-        node0 = i - 1;
-    } else {
-        rA = (ln_slow(xv) - g.U0) * g.inv_dU01;
-    }
-    // ---- rows: one stencil in range, else two probes (rules B, C); row = table row of stencil row 0
-    int row1, row2;
-    double vw1[4], vw2[4];
-    double rB = 0.0;
-    if (high_q) {  // the last two Q^2 knots of the last sub-grid
-        rB = (ln_slow(qv) - g.Va) * g.inv_dVab;
-        row1 = row2 = g.nq_tot - 4;
-        vw1[0] = vw1[1] = vw1[3] = 0.0; vw1[2] = 1.0;
-        vw2[0] = vw2[1] = vw2[2] = 0.0; vw2[3] = 1.0;
-    } else if (low_q) {  // q_min (row 0 of sub-grid 0) and 1.01 q_min (fixed interval and weights)
-        row1 = 0;
-        vw1[0] = 1.0; vw1[1] = vw1[2] = vw1[3] = 0.0;
-        row2 = g.jC - 1;
-#pragma unroll
-        for (int b = 0; b < 4; b++) vw2[b] = g.wvC[b];
-    } else {
-        const double v = ln_slow(qv);
-        const int gi = locate_q(g, sv, qv, v);
-        const IntervalRec32 r = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
-        weights_rec32(r, (v - r.z0) * r.inv_dz, vw1);
-        row1 = row2 = gi - 1;
-    }
-    const bool two_v = high_q || low_q;
-    YW<W> y1 = probe<W>(sv.tab, RB, row1, node0, wu1, vw1, lane8), y2 = y1;
-    if (two_v) y2 = probe<W>(sv.tab, RB, row2, node0, wu1, vw2, lane8);
-    if (low_x) {
-        const YW<W> h1 = probe<W>(sv.tab, RB, row1, 0, wu2, vw1, lane8);
-#pragma unroll
-        for (int k = 0; k < W; k++) y1.v[k] = cont_e(rA, y1.v[k], h1.v[k]);
-        if (two_v) {
-            const YW<W> h2 = probe<W>(sv.tab, RB, row2, 0, wu2, vw2, lane8);
-#pragma unroll
-            for (int k = 0; k < W; k++) y2.v[k] = cont_e(rA, y2.v[k], h2.v[k]);
-        }
-    }
-    const double rho = qv / g.q2_min;
-#pragma unroll
-    for (int k = 0; k < W; k++) {
-        if (high_q) y1.v[k] = cont_e(rB, y1.v[k], y2.v[k]);
-        else if (low_q) y1.v[k] = rule_c(y1.v[k], y2.v[k], rho);
-    }
-    return y1;
-}
-
-// one point's W columns to their output rows (row < 0: column not requested)
-template <int W>
-__device__ __forceinline__ void store_cols(double *__restrict__ out, long long out_stride, long long p,
-                                           const int row[W], const double v[W])
-{
-    if (row[0] >= 0) __stcs(out + row[0] * out_stride + p, v[0]);
-    if (row[1] >= 0) __stcs(out + row[1] * out_stride + p, v[1]);
-    if (W == 4) {
-        if (row[W - 2] >= 0) __stcs(out + row[W - 2] * out_stride + p, v[W - 2]);
-        if (row[W - 1] >= 0) __stcs(out + row[W - 1] * out_stride + p, v[W - 1]);
-    }
-}
-
-// the scale of a point: Q^2, or Q in GeV squared once on load (a non-positive Q is invalid, like Q^2 <= 0)
-template <bool Q_IS_Q>
-__device__ __forceinline__ double load_scale(const double *p)
-{
-    const double q = __ldg(p);
-    return Q_IS_Q ? ((q > 0.0) ? q * q : -1.0) : q;
-}
+#include "xfxq2_slow.cuh"
 
 template <bool Q_IS_Q, int W>  // compile-time: a run-time flag costs 11 % (register pressure at the 128 cap)
 __global__ void __launch_bounds__(NT_SMEM, 1)
@@ -373,7 +36,9 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    __shared__ unsigned char wcnt[NT_SMEM / 32][8];  // entries in each warp's class lists
+    __shared__ unsigned char s_req[NT_SMEM / 32];    // "evaluate your full batches now", one flag per warp
+    const int tid = threadIdx.x, lane = tid & 31;
     // job = (member of the set, pass): blockIdx.x = seq * n_jobs + job; a job's CTAs share its tiles
     const int job = blockIdx.x % n_jobs, seq = blockIdx.x / n_jobs, nseq = gridDim.x / n_jobs;
     const int pass = job % pl.n, mem = job / pl.n;
@@ -387,6 +52,8 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    if (tid < NT_SMEM / 32 * 8) (&wcnt[0][0])[tid] = 0;
+    if (tid < NT_SMEM / 32) s_req[tid] = 0;
     __syncthreads();
     if (tid == 0) {
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(slice_bytes) : "memory");
@@ -418,32 +85,28 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     const bool odd = lane8 & 1;
     const int row[4] = {pl.row[pass][0], pl.row[pass][1], pl.row[pass][2], pl.row[pass][3]};
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
-    // Out-of-grid points are not evaluated where they occur: each warp appends them to one list per
-    // CLASS (0: x < x_min, 1: Q^2 > max, 2: Q^2 < min, 3 and 4: the corners 0+1, 0+2) and evaluates a
-    // list when it holds a warp's worth, so that every slow_point call is class-uniform (no
-    // divergence between the continuation rules) and runs on full lanes.  The lists live in a
-    // global scratch slot owned by this SM (one CTA per SM at a time); counts are warp-uniform,
-    // 6 bits per class in one register.
-    unsigned cnts = 0;
-    constexpr int TILE = NT_SMEM * PPT_SMEM;
-    auto wlist = [&]() -> uint32_t * {
+    // Out-of-grid points are not evaluated where they occur.  Each warp appends their indices to one
+    // list per continuation class (xfxq2_slow.cuh) and evaluates them in whole batches of 32, so that
+    // every call is class-uniform on full lanes; a remainder stays at the front of its list, so batch
+    // k of a class is always the warp's entries 32k .. 32k+31 of that class, whenever it is evaluated
+    // (results do not depend on timing).  WHEN: a warp whose list reaches PDFB_SLOW_TRIGGER entries
+    // advances the CTA's flush epoch; every warp compares the epoch once per tile and evaluates its
+    // full batches when it has moved -- all warps run the out-of-grid code at about the same time,
+    // without a barrier (a barrier every few tiles costs the in-range loop 7-25 %, measured).
+    // The lists live in a global scratch slot owned by this SM: at most one CTA of this kernel is
+    // resident per SM, on any stream, because the launcher requests more than half of the SM's shared
+    // memory (checked at load: occupancy == 1).
+    auto wlist = [&]() -> uint32_t * {  // recomputed where needed: nothing of this lives in a register across the hot loop
         uint32_t smid;
         asm("mov.u32 %0, %%smid;" : "=r"(smid));
-        return g.slow_ws + ((size_t)(smid % PDFB_WS_SLOTS) * (NT_SMEM / 32) + warp) * (PDFB_SLOW_CLASSES * 32);
+        return g.slow_ws + ((size_t)(smid % PDFB_WS_SLOTS) * (NT_SMEM / 32) + (threadIdx.x >> 5)) * (PDFB_SLOW_CLASSES * PDFB_SLOW_LCAP);
     };
-    auto flush = [&](int cls, int count) {
-        __syncwarp();
-        if (lane < count) {
-            const uint32_t e = __ldcg(wlist() + cls * 32 + lane);  // (iteration * PPT + k) << 5 | lane
-            const uint32_t ik = e >> 5;
-            const long long ps = ((long long)seq + (long long)(ik / PPT_SMEM) * nseq) * TILE + (ik % PPT_SMEM) * NT_SMEM +
-                                 warp * 32 + (e & 31);
-            const YW<W> r = slow_point<W>(&g, smem, __ldg(x + ps), load_scale<Q_IS_Q>(q2 + ps), lane8);
-            store_cols<W>(out, out_stride, ps, row, r.v);
-        }
-        __syncwarp();
+    constexpr int TILE = NT_SMEM * PPT_SMEM;
+    auto flush_lists = [&](bool final) {  // warp-uniform
+        flush_warp_lists<Q_IS_Q, W>(final, wlist(), &wcnt[threadIdx.x >> 5][0], &s_req[threadIdx.x >> 5], &g, smem, x, q2, out, out_stride, pl.row[pass]);
     };
 
+    bool pending = false;  // this warp holds at least one full batch (the flush request is only looked at then)
     // software pipeline: the next tile's coordinates are in flight while this tile is evaluated
     long long tile = seq;
     double xv[PPT_SMEM], qv[PPT_SMEM];
@@ -452,7 +115,9 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         const long long p = tile * TILE + k * NT_SMEM + tid;
         xv[k] = (p < n) ? __ldg(x + p) : 1.0; qv[k] = (p < n) ? load_scale<Q_IS_Q>(q2 + p) : 1.0;
     }
-    for (uint32_t it = 0; tile * TILE < n; tile += nseq, ++it) {
+    while (tile * TILE < n) {
+    // the hot loop is left to evaluate class lists (no call inside it: its registers are at the cap)
+    for (; tile * TILE < n; tile += nseq) {
         const long long p0 = tile * TILE + tid;
         double xn[PPT_SMEM], qn[PPT_SMEM];
         bool in_range[PPT_SMEM];
@@ -504,38 +169,52 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                 store_cols<W>(out, out_stride, p, row, nanv);
                 if (job == 0) atomicAdd(g.n_invalid, 1ULL);
             }
-            if (slow_mask) {  // warp-uniform: append the out-of-grid points to their class lists
+            if (slow_mask) {  // warp-uniform: append the out-of-grid points to the warp's class lists
                 const bool low_x = xv[k] < g.x_min, high_q = qv[k] > g.q2_max, low_q = qv[k] < g.q2_min;
                 const int cls = low_x ? (high_q ? 3 : (low_q ? 4 : 0)) : (high_q ? 1 : 2);
-                uint32_t *wl = wlist();
+                const int warp = threadIdx.x >> 5;
+                uint32_t *const wl = wlist();
 #pragma unroll
                 for (int c = 0; c < PDFB_SLOW_CLASSES; c++) {
                     const unsigned m = __ballot_sync(0xffffffffu, slow && cls == c);
                     if (m) {
                         const int kc = __popc(m);
-                        int cur = (cnts >> (6 * c)) & 63;
-                        if (cur + kc > 32) { flush(c, cur); cur = 0; }
+                        const int cur = wcnt[warp][c];
+                        // (cur + kc <= TRIGGER - 1 + 32 + 31 < LCAP: the trigger below empties the list at the end of its tile)
                         if (slow && cls == c)
-                            __stcg(wl + c * 32 + cur + __popc(m & ((1u << lane) - 1u)), ((it * PPT_SMEM + k) << 5) | (uint32_t)lane);
-                        cnts = (cnts & ~(63u << (6 * c))) | ((unsigned)(cur + kc) << (6 * c));
+                            __stcg(wl + c * PDFB_SLOW_LCAP + cur + __popc(m & ((1u << lane) - 1u)), (uint32_t)p);
+                        __syncwarp();
+                        if (lane == 0) wcnt[warp][c] = (unsigned char)(cur + kc);
+                        pending |= (cur + kc >= 32);
+                        // a list reaching the trigger length asks every warp of the CTA to evaluate its batches
+                        if (cur < PDFB_SLOW_TRIGGER && cur + kc >= PDFB_SLOW_TRIGGER && lane < NT_SMEM / 32) s_req[lane] = 1;
                     }
                 }
             }
             xv[k] = xn[k]; qv[k] = qn[k];
         }
+        if (pending && *reinterpret_cast<volatile unsigned char *>(&s_req[threadIdx.x >> 5])) { tile += nseq; break; }
     }
-#pragma unroll
-    for (int c = 0; c < PDFB_SLOW_CLASSES; c++)
-        if ((cnts >> (6 * c)) & 63) flush(c, (cnts >> (6 * c)) & 63);
+    if (pending) { flush_lists(false); pending = false; }
+    }
+    flush_lists(true);
 }
 
-static int smem_needed(const GridDev &d, int W) { return d.pre_bytes + (W == 4 ? d.slice_bytes : d.slice2_bytes) + d.post_bytes; }
-static const int STATIC_SMEM = 256;  // >= the kernel's static shared memory (mbarrier)
+// Dynamic shared memory of a launch.  Never less than PDFB_SMEM_FLOOR (more than half of the SM's
+// 228 KB): two CTAs of this kernel can then not be resident on one SM, whatever the grid size, the
+// register count or the stream -- the invariant the per-SM scratch slot of the class lists rests on.
+static const int PDFB_SMEM_FLOOR = 116 * 1024;
+static int smem_image(const GridDev &d, int W) { return d.pre_bytes + (W == 4 ? d.slice_bytes : d.slice2_bytes) + d.post_bytes; }
+static int smem_needed(const GridDev &d, int W) { const int b = smem_image(d, W); return b > PDFB_SMEM_FLOOR ? b : PDFB_SMEM_FLOOR; }
+static const int STATIC_SMEM = 256;  // >= the kernel's static shared memory (mbarrier, list counters)
+static_assert(NT_SMEM == 512, "PDFB_WS_BYTES and the request flags assume 16 warps per CTA");
+static_assert(PDFB_SLOW_TRIGGER - 1 + 32 + 31 <= 255 && PDFB_SLOW_TRIGGER + 62 <= PDFB_SLOW_LCAP, "8-bit list counters");
 
 // bit 0: the 4-column slices fit the device's shared memory, bit 1: the 2-column slices do
 int pdfb_smem_eligible(const pdfb_grid *g)
 {
     if (getenv("PDFB_FORCE_FALLBACK")) return 0;  // testing: force the read-only-cache path
+    if (g->sms > PDFB_WS_SLOTS) return 0;         // one scratch slot per SM (%smid < %nsmid = the SM count)
     int dev_max = 0;
     if (cudaDeviceGetAttribute(&dev_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, g->device) != cudaSuccess) return 0;
     int ok = 0;
@@ -543,8 +222,9 @@ int pdfb_smem_eligible(const pdfb_grid *g)
     if (smem_needed(g->d, 2) + STATIC_SMEM <= dev_max) ok |= 2;
     if (!ok) return 0;
     // the attribute is per function, not per handle: raise it once to the device maximum
-    static int attr_set_for = -1;
-    if (attr_set_for != g->device) {
+    static std::atomic<unsigned long long> attr_done{0};  // one bit per device; setting twice is harmless
+    const unsigned long long bit = 1ULL << (g->device & 63);
+    if (!(attr_done.load(std::memory_order_acquire) & bit)) {
         const int lim = dev_max - STATIC_SMEM;
         if (cudaFuncSetAttribute(k_xfxq2_smem<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
             cudaFuncSetAttribute(k_xfxq2_smem<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
@@ -553,7 +233,13 @@ int pdfb_smem_eligible(const pdfb_grid *g)
             cudaGetLastError();
             return 0;
         }
-        attr_set_for = g->device;
+        attr_done.fetch_or(bit, std::memory_order_release);
+    }
+    // the scratch-slot invariant, checked rather than assumed: one resident CTA per SM
+    int occ = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfxq2_smem<false, 4>, NT_SMEM, PDFB_SMEM_FLOOR) != cudaSuccess || occ != 1) {
+        cudaGetLastError();
+        return 0;
     }
     return ok;
 }
@@ -596,24 +282,28 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     const bool use2 = !(ok & 1) || ((ok & 2) && 3.6 * pl2.n < 5.6 * pl4.n);
     const PassList &pl = use2 ? pl2 : pl4;
     const int W = use2 ? 2 : 4;
-    int sms = 148;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, g->device);
+    const int sms = g->sms;
     // jobs = (member, pass).  Few jobs: the SMs are split between them and each CTA is persistent
     // over its share of the tiles.  More jobs than SMs: one CTA per job over all tiles, scheduled
     // by the hardware as SMs free up (one CTA per SM at a time: the slice fills shared memory).
     const long long n_jobs = (long long)pl.n * n_mem;
     if (n_jobs > 0x3fffffff) return PDFB_ELIMIT;
-    int per_job = (int)(sms / n_jobs);
-    if (per_job < 1) per_job = 1;
-    long long tiles = (n + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
-    if (per_job > tiles) per_job = (int)tiles;
-    const unsigned grid = (unsigned)(per_job * n_jobs);
     const int smem = smem_needed(g->d, W);
-#define PDFB_LAUNCH(Q, WW) k_xfxq2_smem<Q, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, n, x, q2, out, out_stride, member0, n_req, (int)n_jobs)
-    if (W == 4) { if (q_is_q) PDFB_LAUNCH(true, 4); else PDFB_LAUNCH(false, 4); }
-    else        { if (q_is_q) PDFB_LAUNCH(true, 2); else PDFB_LAUNCH(false, 2); }
+    // the class lists hold point indices as 32-bit offsets: batches beyond 2^31 points go out in slices
+    const long long SLICE = 1LL << 31;
+    for (long long off = 0; off < n; off += SLICE) {
+        const long long m = (n - off < SLICE) ? (n - off) : SLICE;
+        int per_job = (int)(sms / n_jobs);
+        if (per_job < 1) per_job = 1;
+        const long long tiles = (m + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
+        if (per_job > tiles) per_job = (int)tiles;
+        const unsigned grid = (unsigned)(per_job * n_jobs);
+#define PDFB_LAUNCH(Q, WW) k_xfxq2_smem<Q, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, m, x + off, q2 + off, out + off, out_stride, member0, n_req, (int)n_jobs)
+        if (W == 4) { if (q_is_q) PDFB_LAUNCH(true, 4); else PDFB_LAUNCH(false, 4); }
+        else        { if (q_is_q) PDFB_LAUNCH(true, 2); else PDFB_LAUNCH(false, 2); }
 #undef PDFB_LAUNCH
-    pdfb_count_launch(1);
+        pdfb_count_launch(1);
+    }
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;
 }
