@@ -37,7 +37,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar;
     __shared__ unsigned char wcnt[NT_SMEM / 32][8];  // entries in each warp's class lists
-    __shared__ unsigned char s_req[NT_SMEM / 32];    // "evaluate your full batches now", one flag per warp
+    __shared__ __align__(16) unsigned char s_req[NT_SMEM / 32];  // "evaluate your full batches now", one flag per warp
     const int tid = threadIdx.x, lane = tid & 31;
     // job = (member of the set, pass): blockIdx.x = seq * n_jobs + job; a job's CTAs share its tiles
     const int job = blockIdx.x % n_jobs, seq = blockIdx.x / n_jobs, nseq = gridDim.x / n_jobs;
@@ -106,7 +106,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         flush_warp_lists<Q_IS_Q, W>(final, wlist(), &wcnt[threadIdx.x >> 5][0], &s_req[threadIdx.x >> 5], &g, smem, x, q2, out, out_stride, pl.row[pass]);
     };
 
-    bool pending = false;  // this warp holds at least one full batch (the flush request is only looked at then)
+    bool pending = false;  // this warp has list entries (the flush request is only looked at then)
     // software pipeline: the next tile's coordinates are in flight while this tile is evaluated
     long long tile = seq;
     double xv[PPT_SMEM], qv[PPT_SMEM];
@@ -131,7 +131,6 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         }
         if (any_in) {
             // ---- locate (LUT guess + exact comparisons where needed), weights, one gather per point.
-            // A lane whose point is out of range computes a dummy in-range point and stores nothing.
 #pragma unroll
             for (int k = 0; k < PPT_SMEM; k++) {
                 const double xs = in_range[k] ? xv[k] : g.x_min, qs = in_range[k] ? qv[k] : g.q2_min;
@@ -161,7 +160,6 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
             const bool live = p < n;
             const bool invalid = live && !in_range[k] && (!(xv[k] > 0.0) || !(qv[k] > 0.0) || !(xv[k] <= g.x_max) || isinf(qv[k]));
             const bool slow = live && !in_range[k] && !invalid;
-            const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
             if (invalid) {
                 double nanv[W];
 #pragma unroll
@@ -169,27 +167,25 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                 store_cols<W>(out, out_stride, p, row, nanv);
                 if (job == 0) atomicAdd(g.n_invalid, 1ULL);
             }
+            const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
             if (slow_mask) {  // warp-uniform: append the out-of-grid points to the warp's class lists
-                const bool low_x = xv[k] < g.x_min, high_q = qv[k] > g.q2_max, low_q = qv[k] < g.q2_min;
-                const int cls = low_x ? (high_q ? 3 : (low_q ? 4 : 0)) : (high_q ? 1 : 2);
-                const int warp = threadIdx.x >> 5;
-                uint32_t *const wl = wlist();
-#pragma unroll
-                for (int c = 0; c < PDFB_SLOW_CLASSES; c++) {
-                    const unsigned m = __ballot_sync(0xffffffffu, slow && cls == c);
-                    if (m) {
-                        const int kc = __popc(m);
-                        const int cur = wcnt[warp][c];
-                        // (cur + kc <= TRIGGER - 1 + 32 + 31 < LCAP: the trigger below empties the list at the end of its tile)
-                        if (slow && cls == c)
-                            __stcg(wl + c * PDFB_SLOW_LCAP + cur + __popc(m & ((1u << lane) - 1u)), (uint32_t)p);
-                        __syncwarp();
-                        if (lane == 0) wcnt[warp][c] = (unsigned char)(cur + kc);
-                        pending |= (cur + kc >= 32);
+                if (slow) {
+                    const bool low_x = xv[k] < g.x_min, high_q = qv[k] > g.q2_max, low_q = qv[k] < g.q2_min;
+                    const int cls = low_x ? (high_q ? 3 : (low_q ? 4 : 0)) : (high_q ? 1 : 2);
+                    const unsigned peers = __match_any_sync(slow_mask, cls);  // the lanes of this class
+                    unsigned char *cnt = &wcnt[threadIdx.x >> 5][cls];
+                    const int cur = *cnt, kc = __popc(peers);
+                    // (cur + kc <= TRIGGER - 1 + 32 + 31 < LCAP: the trigger below empties the list at the end of its tile)
+                    __stcg(wlist() + cls * PDFB_SLOW_LCAP + cur + __popc(peers & ((1u << lane) - 1u)), (uint32_t)p);
+                    __syncwarp(slow_mask);
+                    if ((peers & ((1u << lane) - 1u)) == 0) {  // the first lane of the class
+                        *cnt = (unsigned char)(cur + kc);
                         // a list reaching the trigger length asks every warp of the CTA to evaluate its batches
-                        if (cur < PDFB_SLOW_TRIGGER && cur + kc >= PDFB_SLOW_TRIGGER && lane < NT_SMEM / 32) s_req[lane] = 1;
+                        if (cur < PDFB_SLOW_TRIGGER && cur + kc >= PDFB_SLOW_TRIGGER)
+                            *reinterpret_cast<uint4 *>(s_req) = make_uint4(0x01010101u, 0x01010101u, 0x01010101u, 0x01010101u);
                     }
                 }
+                pending = true;  // (looked at together with the request flag; cleared by the flush)
             }
             xv[k] = xn[k]; qv[k] = qn[k];
         }

@@ -226,11 +226,16 @@ template <int W>
 __device__ __forceinline__ void store_cols(double *__restrict__ out, long long out_stride, long long p,
                                            const int row[W], const double v[W])
 {
-    if (row[0] >= 0) __stcs(out + row[0] * out_stride + p, v[0]);
-    if (row[1] >= 0) __stcs(out + row[1] * out_stride + p, v[1]);
+#ifdef PDFB_STORE_DEFAULT
+#define PDFB_ST(ptr, val) (*(ptr) = (val))
+#else
+#define PDFB_ST(ptr, val) __stcs(ptr, val)
+#endif
+    if (row[0] >= 0) PDFB_ST(out + row[0] * out_stride + p, v[0]);
+    if (row[1] >= 0) PDFB_ST(out + row[1] * out_stride + p, v[1]);
     if (W == 4) {
-        if (row[W - 2] >= 0) __stcs(out + row[W - 2] * out_stride + p, v[W - 2]);
-        if (row[W - 1] >= 0) __stcs(out + row[W - 1] * out_stride + p, v[W - 1]);
+        if (row[W - 2] >= 0) PDFB_ST(out + row[W - 2] * out_stride + p, v[W - 2]);
+        if (row[W - 1] >= 0) PDFB_ST(out + row[W - 1] * out_stride + p, v[W - 1]);
     }
 }
 
