@@ -52,12 +52,13 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
 }
 
 // Fast path (K <= 192 nodes): replicated coefficient lines in shared memory, LUT location,
-// one cubic in t per point.  Two points per thread keep two independent ln chains in flight.
+// one cubic in t per point, ln Q^2 through a 64-entry table (ln_tab, pdfb_internal.cuh).  Four points per
+// thread and iteration; 3 CTAs of 512 threads per SM (48 KB of tables each).
 #ifndef NT_ALPHAS
 #define NT_ALPHAS 512
 #endif
 #ifndef CTAS_ALPHAS
-#define CTAS_ALPHAS 2
+#define CTAS_ALPHAS 3
 #endif
 
 template <bool Q_IS_Q>
@@ -70,6 +71,7 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
         reinterpret_cast<int4 *>(smem)[e] = __ldg(reinterpret_cast<const int4 *>(A.fast) + e);
     __syncthreads();
     const uint32_t lines = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)((threadIdx.x & 7) << 4);
+    const uint32_t lntab = lines + (uint32_t)A.f_lntab;
     const double *q2k = reinterpret_cast<const double *>(smem + A.f_q2k);
     const unsigned short *lut = reinterpret_cast<const unsigned short *>(smem + A.f_lut);
     const double qnan = __longlong_as_double(0x7ff8000000000000LL);
@@ -77,7 +79,9 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
         double res;
         if (Q_IS_Q) qv = (qv > 0.0) ? qv * qv : -1.0;  // Q in GeV -> Q^2
         if (qv >= A.q2_min && qv <= A.q2_max) {
-            const double v = pdfb_ln(qv);
+            double2 le;  // {1/c, ln c} of qv's mantissa bin
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(le.x), "=d"(le.y) : "r"(lntab + (uint32_t)ln_tab_bin(qv) * 128u));
+            const double v = ln_tab(qv, le);
             int b = min(max((int)((v - A.lut_v0) * A.lut_inv_h), 0), PDFB_LUT_BINS - 1);
             const int e = lut[b], d = (e >> 1) & 3;
             int m = e >> 3;
@@ -85,7 +89,7 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
             if (e & 1)
                 while (m < A.K - 1 && q2k[m + 1] <= qv) ++m;
             m = min(m, A.K - 2);  // Q^2 = last node: last interval, t = 1
-            const uint32_t rec = lines + (uint32_t)m * 512u;
+            const uint32_t rec = lines + (uint32_t)m * (uint32_t)PDFB_ALPHAS_LINE;
             double2 zi, c01, c23;
             asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(zi.x), "=d"(zi.y) : "r"(rec));
             asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(c01.x), "=d"(c01.y) : "r"(rec + 128u));

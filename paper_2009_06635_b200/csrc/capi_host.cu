@@ -51,9 +51,10 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
     d.a_first = alphas[0]; d.a_last = alphas[n_knots - 1];
 
     size_t o_q2 = 0, o_a = align_up(sizeof(double) * n_knots, 128), o_z = 2 * o_a, o_rec = 3 * o_a;
-    // fast-path block: [lines K*512][q2k K doubles][lut u16]
+    // fast-path block: [lines K*384][ln table][q2k K doubles][lut u16]
     d.fast_ok = (n_knots <= 192);
-    d.f_q2k = 512 * n_knots;
+    d.f_lntab = PDFB_ALPHAS_LINE * n_knots;
+    d.f_q2k = d.f_lntab + PDFB_LNTAB_BYTES;
     d.f_lut = d.f_q2k + (int)sizeof(double) * n_knots;
     d.fast_bytes = (int)align_up(d.f_lut + 2 * PDFB_LUT_BINS, 16);
     size_t o_fast = align_up(o_rec + sizeof(IntervalRec) * n_knots, 128);
@@ -67,8 +68,17 @@ extern "C" int alphas_grid_load(int n_knots, const double *q_knots, const double
         rc = PDFB_ECUDA;
     if (!rc) rc = pdfb_setup_ln((const double *)(blob + o_q2), (double *)(blob + o_z), n_knots, 0);
     if (!rc) rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_rec), nullptr, n_sub, d.off, 0);
+    if (!rc) {  // ln table of the fast path: entry j = {1/c_j, ln c_j}, c_j = 1 + (j + 1/2)/64, 8 copies per line
+        std::vector<double> tab(PDFB_LNTAB_BYTES / 8);
+        for (int j = 0; j < 64; j++) {
+            const double c = 1.0 + (j + 0.5) / 64.0;
+            for (int k = 0; k < 8; k++) { tab[(j * 8 + k) * 2] = 1.0 / c; tab[(j * 8 + k) * 2 + 1] = std::log(c); }
+        }
+        if (cudaMemcpy(blob + o_fast + d.f_lntab, tab.data(), PDFB_LNTAB_BYTES, cudaMemcpyHostToDevice) != cudaSuccess) rc = PDFB_ECUDA;
+    }
     if (!rc) rc = pdfb_setup_alphas_fast((const IntervalRec *)(blob + o_rec), (const double *)(blob + o_a),
-                                         (unsigned char *)(blob + o_fast), n_sub, d.off, 0);
+                                         (const double *)(blob + o_q2), (unsigned char *)(blob + o_fast),
+                                         (const double2 *)(blob + o_fast + d.f_lntab), n_sub, d.off, 0);
     if (!rc && cudaMemcpy(h_z.data(), blob + o_z, sizeof(double) * n_knots, cudaMemcpyDeviceToHost) != cudaSuccess) rc = PDFB_ECUDA;
     if (!rc) {  // LUT over ln Q^2 (encoding in pdfb_internal.cuh); a repeated node lands on its upper copy
         std::vector<unsigned short> lut(PDFB_LUT_BINS);

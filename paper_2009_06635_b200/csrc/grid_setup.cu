@@ -140,14 +140,18 @@ int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off,
 
 // alpha_s fast-path records: cubic coefficients of each interval in t, from the O2 records.
 // p(t) = h00 y0 + h10 dL + h01 y1 + h11 dH = y0 + dL t + (3(y1-y0) - 2 dL - dH) t^2 + (dL + dH - 2(y1-y0)) t^3
+// (the fast path takes its logarithms with ln_tab, pdfb_internal.cuh: the node logarithm stored here
+// comes from the same function, so that a query on a node gets t = 0 exactly)
 __global__ void k1_alphas_lines(const IntervalRec *__restrict__ rec, const double *__restrict__ a,
-                                unsigned char *__restrict__ lines, int lo, int M)
+                                const double *__restrict__ q2k, unsigned char *__restrict__ lines,
+                                const double2 *__restrict__ lntab, int lo, int M)
 {
     int m = blockIdx.x * blockDim.x + threadIdx.x;  // interval m of the sub-grid [lo, lo+M)
     if (m >= M) return;
-    double chunk[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    double chunk[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
     const IntervalRec r = rec[lo + m];
-    chunk[0][0] = r.z0; chunk[0][1] = r.inv_dz;
+    const double q = q2k[lo + m];
+    chunk[0][0] = ln_tab(q, lntab[ln_tab_bin(q) * 8]); chunk[0][1] = r.inv_dz;
     if (m < M - 1) {
         const double y0 = a[lo + m], y1 = a[lo + m + 1];
         const double ym = a[lo + max(m - 1, 0)], yp = a[lo + min(m + 2, M - 1)];
@@ -158,17 +162,17 @@ __global__ void k1_alphas_lines(const IntervalRec *__restrict__ rec, const doubl
         chunk[2][0] = 3.0 * dy - 2.0 * dL - dH;
         chunk[2][1] = dL + dH - 2.0 * dy;
     }
-    double2 *dst = reinterpret_cast<double2 *>(lines + (size_t)(lo + m) * 512);
-    for (int k = 0; k < 4; k++)
+    double2 *dst = reinterpret_cast<double2 *>(lines + (size_t)(lo + m) * PDFB_ALPHAS_LINE);
+    for (int k = 0; k < 3; k++)
         for (int c = 0; c < 8; c++) dst[k * 8 + c] = make_double2(chunk[k][0], chunk[k][1]);
 }
 
-int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, unsigned char *d_lines, int n_sub,
-                           const int *h_off, cudaStream_t st)
+int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, const double *d_q2k, unsigned char *d_lines,
+                           const double2 *d_lntab, int n_sub, const int *h_off, cudaStream_t st)
 {
     for (int s = 0; s < n_sub; s++) {
         int M = h_off[s + 1] - h_off[s];
-        k1_alphas_lines<<<(M + 63) / 64, 64, 0, st>>>(d_rec, d_a, d_lines, h_off[s], M);
+        k1_alphas_lines<<<(M + 63) / 64, 64, 0, st>>>(d_rec, d_a, d_q2k, d_lines, d_lntab, h_off[s], M);
         pdfb_count_launch(1);
     }
     PDFB_CUDA(cudaGetLastError());

@@ -101,6 +101,33 @@ __device__ __forceinline__ double pdfb_ln(double a)
     return (a >= 2.2250738585072014e-308) ? ln_pos(a) : log(a);
 }
 
+// ---------------------------------------------------------------------------------------------
+// ln of a positive normal double through a 64-entry table (alpha_s fast path, alphas_kernels.cu):
+// a = 2^k m, m in [1, 2); c = 1 + (j + 1/2)/64 the centre of m's bin j (the top 6 mantissa bits);
+// ln a = k ln2 + ln c + log1p(m/c - 1), |m/c - 1| < 2^-7, series to the 7th power (remainder < 2^-59).
+// Absolute error a few 1e-16 + |k| ulp-level terms: ~1e-15 at |ln a| ~ 25.  alpha_s(t) moves by at
+// most ~0.1 alpha per unit t = (ln Q^2 - Z_m)/dZ, so the 1e-12 rule needs |error of ln| < 1e-11 dZ:
+// four orders of magnitude to spare on any sensible node list -- and less than half the instructions
+// of ln_pos (no reciprocal).  The node logarithms of the fast path are taken with the same function,
+// so a query on a node still gets t = 0 exactly.  Table entry = {1/c, ln c}, 8 copies per 128-byte
+// line (a lane reads copy lane & 7: conflict-free).
+#define PDFB_LNTAB_BYTES (64 * 128)
+__device__ __forceinline__ int ln_tab_bin(double a) { return (__double2hiint(a) >> 14) & 63; }
+__device__ __forceinline__ double ln_tab(double a, double2 e)
+{
+    const int hi = __double2hiint(a);
+    const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(a));
+    const double kf = (double)((hi >> 20) - 1023);
+    const double r = fma(m, e.x, -1.0);
+    double p = fma(r, 1.0 / 7.0, -1.0 / 6.0);
+    p = fma(p, r, 0.2);
+    p = fma(p, r, -0.25);
+    p = fma(p, r, 1.0 / 3.0);
+    p = fma(p, r, -0.5);
+    p = fma(p * r, r, r);  // log1p(r)
+    return fma(kf, c_ln[0], (e.y + fma(kf, c_ln[1], p)));
+}
+
 struct GridDev {
     int n_sub, nx, n_pid, nq_tot;
     int n_members;                     // member tables sharing these knots (pdf_set_load)
@@ -174,12 +201,12 @@ struct AlphasDev {
     const double *q2k;        // [K]
     const double *a;          // [K]
     const IntervalRec *rec;   // [K]
-    // fast path (alphas_kernels.cu): per interval 4 lines of 128 B; line k = the 16-byte chunk k of
-    // {ln knot, 1/d | c0, c1 | c2, c3 | pad} repeated 8 times, so lane l reads slot (l & 7) of each
+    // fast path (alphas_kernels.cu): per interval 3 lines of 128 B; line k = the 16-byte chunk k of
+    // {ln knot, 1/d | c0, c1 | c2, c3} repeated 8 times, so lane l reads slot (l & 7) of each
     // line: conflict-free whatever intervals the lanes want.  alpha_s(t) = c0 + t(c1 + t(c2 + t c3)).
     int fast_ok;
-    const unsigned char *fast;  // [lines: K*512 B][q2k: K doubles][lut: PDFB_LUT_BINS u16]
-    int fast_bytes, f_q2k, f_lut;
+    const unsigned char *fast;  // [lines: K*384 B][ln table: PDFB_LNTAB_BYTES][q2k: K doubles][lut: PDFB_LUT_BINS u16]
+    int fast_bytes, f_lntab, f_q2k, f_lut;
     double lut_v0, lut_inv_h;
 };
 
@@ -242,8 +269,9 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
                            const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
                            int member0, int n_mem);
 int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st);
-int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, unsigned char *d_lines, int n_sub,
-                            const int *h_off, cudaStream_t st);
+int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, const double *d_q2k, unsigned char *d_lines,
+                           const double2 *d_lntab, int n_sub, const int *h_off, cudaStream_t st);
+#define PDFB_ALPHAS_LINE 384   // bytes per interval in the fast-path image
 int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
                       cudaStream_t st);
 

@@ -59,6 +59,25 @@ def test_alphas_general_kernel_300_nodes(torch_cuda):
         B.load_alphas_spec(W.make_alphas_grid(nq_per_sub=(32, 64, 160, 257)))
 
 
+def test_alphas_fast_path_dense_nodes(torch_cuda):
+    """The replicated-line fast path (<= 192 nodes) with its table-based logarithm on a dense list:
+    190 nodes, i.e. ln Q^2 spacings down to 0.02 (the tolerance budget of that logarithm scales with
+    the spacing, pdfb_internal.cuh); nodes, their neighbours, thresholds with jumps, outside."""
+    torch = torch_cuda
+    aspec = W.make_alphas_grid(nq_per_sub=(40, 50, 50, 50), jump=(1.0, 0.97, 1.01, 1.03))
+    assert len(aspec.q_knots) == 190
+    assert np.diff(np.log(aspec.q_knots[:40] ** 2)).min() < 0.025
+    ha = B.load_alphas_spec(aspec)
+    q2 = _alphas_points(aspec, np.random.default_rng(9), 400_003)
+    dq = torch.from_numpy(q2).cuda()
+    out = torch.empty_like(dq)
+    B.alphas_q2(ha, dq, out)
+    torch.cuda.synchronize()
+    st = check_parity(out.cpu().numpy(), oracle.OracleAlphas.from_spec(aspec).q2(q2), what="alphas 190 nodes (fast path)")
+    assert st["n_clause"] == 0 and st["max_eq1"] < 2e-13
+    B.alphas_grid_free(ha)
+
+
 @pytest.mark.parametrize("nodes", [(6, 12, 30, 52), (20, 40, 100, 140)])
 def test_alphas_q2_host_entry(torch_cuda, nodes):
     """alphas_q2_host (host buffers, chunked pipeline): bit-identical to alphas_q2 on the same
