@@ -45,6 +45,7 @@ enum {
 #define PDFB_MAX_SUBGRIDS 16
 #define PDFB_MAX_PIDS 32
 #define PDFB_MAX_MEMBERS 4096
+#define PDFB_LUMI_MAXF 14   /* pdf_lumi_events: at most this many PIDs in the grid */
 
 /*
  * pdf_grid_load -- upload one PDF member's knot grid and run the grid-setup kernel
@@ -171,6 +172,34 @@ int alphas_q2_host(pdfb_alphas *a, long long n, const double *q2, double *out);
 void alphas_grid_free(pdfb_alphas *a);
 
 const char *pdfb_strerror(int code);
+
+/*
+ * pdf_lumi_events -- the fused call for Monte-Carlo integrands.  An event of a
+ * hadron-collider integrand carries the momentum fractions of the two beams and ONE factorisation
+ * scale (section 4.1; section 4.2; "events of the order of 10^6
+ * at once"); what the integrand needs from the PDF is the parton luminosity
+ *
+ *   lumi[e] = sum_{t < n_terms} coeff[t] * xf(pid_a[t]; x1[e], q2[e]) * xf(pid_b[t]; x2[e], q2[e])
+ *
+ * with xf exactly the value pdf_xfxq2 returns (in range and outside the grid alike).  One call
+ * replaces pdf_xfxq2(x1), pdf_xfxq2(x2), the caller's contraction and, if `a` is given, alphas_q2 on
+ * the same scales: ln Q^2, the Q^2 interval and its weights are taken once per event, and 8 (16)
+ * bytes per event are written instead of 176.
+ *   a, alphas_out  both NULL, or an alpha_s handle of the same device and a device array [n] that
+ *                  receives alpha_s(q2[e])
+ *   n_terms, pid_a, pid_b, coeff   host arrays [n_terms]: the flavour-pair table c_ab as a list of
+ *                  terms (PID 0 = 21; a pair may appear more than once: coefficients add up); every
+ *                  PID must be in the grid (PDFB_EPID), every coefficient finite
+ *   x1, x2, q2     device [n]
+ *   lumi           device [n]; NaN where either point has no value (x > x_max, x <= 0, Q^2 <= 0, NaN;
+ *                  counted by pdf_grid_status, once per event)
+ *   flags          bit 0: divide by x1[e] * x2[e] (the luminosity of f = xf / x)
+ * Member 0 of a set.  Grids with more than PDFB_LUMI_MAXF PIDs: PDFB_ELIMIT.  Allocates nothing,
+ * never synchronises, enqueues two or three kernels on `cuda_stream`.
+ */
+int pdf_lumi_events(const pdfb_grid *g, const pdfb_alphas *a, int n_terms, const int *pid_a, const int *pid_b,
+                    const double *coeff, long long n, const double *x1, const double *x2, const double *q2,
+                    double *lumi, double *alphas_out, int flags, void *cuda_stream);
 
 /* Diagnostic: out[i] = the library's coordinate logarithm of in[i] (device pointers, in > 0).
  * Every ln of a knot or of a query coordinate goes through this one function (R-ln). */

@@ -158,3 +158,32 @@ def xfxq2_members(x_knots, q_offsets, q_knots, grid_pids, member_values, pids, x
     if with_scale:
         return np.stack(outs), np.stack(scales)
     return np.stack(outs)
+
+
+def lumi_events(og1, terms, x1, x2, q2, og2=None, divide_by_x: bool = False, with_scale: bool = False):
+    """Parton luminosity of Monte-Carlo events (x1, x2 and one shared Q^2
+    per event): L[e] = sum_t c_t * xf_{a_t}(x1[e], Q2[e]) * xf_{b_t}(x2[e], Q2[e]) -- the definition
+    written out: the single-point oracle twice, then the sum over the terms in list order.
+    ``og2`` (default: og1) takes the second beam's values from another grid (used by the bilinearity pin).
+    with_scale also returns S = sum_t |c_t| (S_a |xf_b| + |xf_a| S_b), the first-order conditioning scale
+    of the sum (S_a, S_b the scales of the two factors; tolerance helper only)."""
+    og2 = og1 if og2 is None else og2
+    terms = [(int(a), int(b), float(c)) for a, b, c in terms]
+    pa = sorted({t[0] for t in terms})
+    pb = sorted({t[1] for t in terms})
+    r1 = og1.xfxq2(pa, x1, q2, with_scale=with_scale)
+    r2 = og2.xfxq2(pb, x2, q2, with_scale=with_scale)
+    f1, s1 = r1 if with_scale else (r1, None)
+    f2, s2 = r2 if with_scale else (r2, None)
+    lum = np.zeros(len(np.atleast_1d(x1)), dtype=np.float64)
+    sc = np.zeros_like(lum)
+    for a, b, c in terms:
+        ia, ib = pa.index(a), pb.index(b)
+        lum = lum + c * (f1[ia] * f2[ib])
+        if with_scale:
+            sc = sc + abs(c) * (s1[ia] * np.abs(f2[ib]) + np.abs(f1[ia]) * s2[ib])
+    if divide_by_x:
+        d = np.asarray(x1, dtype=np.float64) * np.asarray(x2, dtype=np.float64)
+        lum = lum / d
+        sc = sc / np.abs(d)
+    return (lum, sc) if with_scale else lum

@@ -22,7 +22,7 @@ _ll = ctypes.c_longlong
 
 EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
-           "pdfb_launch_count", "pdfb_probe", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
+           "pdfb_launch_count", "pdfb_probe", "pdf_lumi_events", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
            "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
 
 
@@ -55,6 +55,8 @@ def lib():
         L.pdf_xfxq2_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq_members.restype = ctypes.c_int
         L.pdf_xfxq_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
+        L.pdf_lumi_events.restype = ctypes.c_int
+        L.pdf_lumi_events.argtypes = [_vp, _vp, ctypes.c_int, _ip, _ip, _dp, _ll, _vp, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]
         L.pdf_xfxq2.restype = ctypes.c_int
         L.pdf_xfxq2.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq.restype = ctypes.c_int
@@ -220,6 +222,21 @@ def pdf_xfxq2(g, pids, x, q2, out, stream=None, n=None):
     rc = lib().pdf_xfxq2(_vp(g), len(pids), pids.ctypes.data_as(_ip), n, _dev_ptr(x, n, "x"),
                          _dev_ptr(q2, n, "q2"), _dev_ptr(out, len(pids) * n, "out"), _stream_ptr(stream))
     _check(rc, "pdf_xfxq2")
+
+
+def pdf_lumi_events(g, terms, x1, x2, q2, lumi, alphas=None, alphas_out=None, divide_by_x=False, stream=None, n=None):
+    """Enqueue the fused parton luminosity sum_t c_t xf_a(x1,Q2) xf_b(x2,Q2) for device tensors -> lumi[n]
+    (and alpha_s(Q2) -> alphas_out[n] if an alpha_s handle is given).  terms: iterable of (pid_a, pid_b, c)."""
+    terms = list(terms)
+    pa, pb = _i32([t[0] for t in terms]), _i32([t[1] for t in terms])
+    cc = _f64([t[2] for t in terms])
+    n = int(x1.numel() if n is None else n)
+    rc = lib().pdf_lumi_events(_vp(g), _vp(alphas) if alphas is not None else None, len(terms), pa.ctypes.data_as(_ip),
+                               pb.ctypes.data_as(_ip), cc.ctypes.data_as(_dp), n, _dev_ptr(x1, n, "x1"), _dev_ptr(x2, n, "x2"),
+                               _dev_ptr(q2, n, "q2"), _dev_ptr(lumi, n, "lumi"),
+                               _dev_ptr(alphas_out, n, "alphas_out") if alphas_out is not None else None,
+                               1 if divide_by_x else 0, _stream_ptr(stream))
+    _check(rc, "pdf_lumi_events")
 
 
 def pdf_xfxq(g, pids, x, q, out, stream=None, n=None):

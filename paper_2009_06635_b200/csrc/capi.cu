@@ -246,6 +246,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.aux = (const unsigned char *)(blob + o_aux);
     d.slow_ws = (uint32_t *)(blob + o_ws);
     if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
+    pdfb_lumi_plan(g);
     *out = g;
     return PDFB_OK;
 }

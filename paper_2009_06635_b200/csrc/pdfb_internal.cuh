@@ -210,6 +210,14 @@ struct AlphasDev {
     double lut_v0, lut_inv_h;
 };
 
+// pdf_lumi_events (lumi_kernels.cu): shared-memory plan of the band kernel
+struct LumiLayout {
+    int R, R_alloc, CB, n_bands, ncell;
+    int RB2;          // bytes per row of a 2-column slice
+    int pair_stride;  // bytes between the bands of two pairs in shared memory (a multiple of 128)
+    int l_band, l_qrec, l_list, total;
+};
+
 // Makes the handle's device current for the duration of a call and puts the caller's device back.
 struct DeviceGuard {
     int prev = -1;
@@ -226,6 +234,8 @@ struct DeviceGuard {
 struct pdfb_grid {
     int device;
     int sms;                  // multiprocessors of `device`
+    LumiLayout lumi;          // band plan of pdf_lumi_events
+    int lumi_npair;           // its kernel instance (column pairs staged per band); 0 = general kernel only
     GridDev d;
     int pids[PDFB_MAX_PIDS];
     void *blob;               // one device allocation holding all tables
@@ -265,6 +275,7 @@ int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_r
 int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
                             int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W = 4);
 int pdfb_smem_eligible(const pdfb_grid *g);
+int pdfb_lumi_plan(pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
                            const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
                            int member0, int n_mem);

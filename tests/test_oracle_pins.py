@@ -635,3 +635,44 @@ def test_member_set_is_linear_in_the_tables():
     for m in range(3):
         single = oracle.OraclePdfGrid(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tabs[m]).xfxq2(pids, x, q2)
         assert np.array_equal(single, out[m])
+
+
+# ----------------------------------------------------------------------------------
+# Parton luminosity of events: the helper is "the single-point oracle
+# twice, then the sum over the terms"; pinned by what the mathematics fixes -- in range it is
+# BILINEAR in the tables of the two beams, a single term is the product of two single values, and
+# exchanging the beams together with the pair table changes nothing.
+# ----------------------------------------------------------------------------------
+def test_lumi_helper_is_bilinear_and_symmetric():
+    rng = np.random.default_rng(43)
+    xk = rand_knots(rng, 1e-5, 1.0, 9)
+    subs = [rand_knots(rng, 1.5, 4.0, 5), rand_knots(rng, 4.0, 90.0, 6)]
+    pids = [-1, 1, 2, 21]
+    size = sum(len(xk) * len(q) * len(pids) for q in subs)
+    spec = make_spec(xk, subs, pids, values=[np.zeros((len(xk), len(q), len(pids))) for q in subs])
+
+    def og(tab):
+        return oracle.OraclePdfGrid(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, tab)
+
+    t1, t2, t3 = rng.normal(size=size), rng.normal(size=size), rng.normal(size=size)
+    a, b = 0.5, -1.75
+    n = 400
+    x1 = np.exp(rng.uniform(np.log(xk[0]), 0.0, n)); x2 = np.exp(rng.uniform(np.log(xk[0]), 0.0, n))
+    q2 = np.exp(rng.uniform(np.log(spec.q2_min), np.log(spec.q2_max), n))
+    terms = [(1, -1, 1.0), (-1, 1, 1.0), (21, 21, 0.3), (2, 0, -0.7), (2, 21, 0.1)]   # PID 0 = 21; (2,21) appears twice
+    L = lambda g1, g2: oracle.lumi_events(g1, terms, x1, x2, q2, og2=g2, with_scale=True)
+    l13, s13 = L(og(t1), og(t3)); l23, s23 = L(og(t2), og(t3)); lc3, _ = L(og(a * t1 + b * t2), og(t3))
+    assert np.all(np.abs(lc3 - (a * l13 + b * l23)) <= 4e-15 * (abs(a) * s13 + abs(b) * s23) + 1e-300)
+    l31, s31 = L(og(t3), og(t1)); l32, s32 = L(og(t3), og(t2)); l3c, _ = L(og(t3), og(a * t1 + b * t2))
+    assert np.all(np.abs(l3c - (a * l31 + b * l32)) <= 4e-15 * (abs(a) * s31 + abs(b) * s32) + 1e-300)
+    # one term with unit coefficient = the product of the two single-point values, bit for bit
+    g1 = og(t1)
+    single = oracle.lumi_events(g1, [(2, -1, 1.0)], x1, x2, q2)
+    assert np.array_equal(single, g1.xfxq2([2], x1, q2)[0] * g1.xfxq2([-1], x2, q2)[0])
+    # exchanging the beams and transposing the pair table changes nothing but the summation order
+    swapped = oracle.lumi_events(g1, [(b_, a_, c) for a_, b_, c in terms], x2, x1, q2)
+    direct, sc = oracle.lumi_events(g1, terms, x1, x2, q2, with_scale=True)
+    assert np.all(np.abs(swapped - direct) <= 4e-16 * sc + 1e-300)
+    # the 1/(x1 x2) form, and the scale bounds the sum of term magnitudes
+    assert np.allclose(oracle.lumi_events(g1, terms, x1, x2, q2, divide_by_x=True), direct / (x1 * x2), rtol=4e-16, atol=0)
+    assert np.all(np.abs(direct) <= sc * (1 + 1e-12))
