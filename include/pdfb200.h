@@ -174,6 +174,20 @@ void alphas_grid_free(pdfb_alphas *a);
 const char *pdfb_strerror(int code);
 
 /*
+ * pdf_xfxq2_pm, pdf_xfxq2_f32 -- pdf_xfxq2 with another output layout / precision (
+ * the interpolating methods of the PDF object).  Same arguments, same arithmetic (fp64),
+ * same error behaviour as pdf_xfxq2; compile-time variants of the same kernels.
+ *   pdf_xfxq2_pm   out: device double [n][n_req], point-major: out[p*n_req + r] (all flavours of an
+ *                  event next to each other, the layout an event loop reads)
+ *   pdf_xfxq2_f32  out: device float [n_req][n], flavour-major: the fp64 result rounded ONCE to fp32 at
+ *                  the store (half the output bytes; NaN where no value is defined)
+ */
+int pdf_xfxq2_pm(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                 const double *q2, double *out, void *cuda_stream);
+int pdf_xfxq2_f32(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                  const double *q2, float *out, void *cuda_stream);
+
+/*
  * pdf_lumi_events -- the fused call for Monte-Carlo integrands.  An event of a
  * hadron-collider integrand carries the momentum fractions of the two beams and ONE factorisation
  * scale (section 4.1; section 4.2; "events of the order of 10^6

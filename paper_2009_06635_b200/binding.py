@@ -22,7 +22,7 @@ _ll = ctypes.c_longlong
 
 EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
-           "pdfb_launch_count", "pdfb_probe", "pdf_lumi_events", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
+           "pdfb_launch_count", "pdfb_probe", "pdf_lumi_events", "pdf_xfxq2_pm", "pdf_xfxq2_f32", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
            "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
 
 
@@ -55,6 +55,9 @@ def lib():
         L.pdf_xfxq2_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_xfxq_members.restype = ctypes.c_int
         L.pdf_xfxq_members.argtypes = [_vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
+        for fn in (L.pdf_xfxq2_pm, L.pdf_xfxq2_f32):
+            fn.restype = ctypes.c_int
+            fn.argtypes = [_vp, ctypes.c_int, _ip, _ll, _vp, _vp, _vp, _vp]
         L.pdf_lumi_events.restype = ctypes.c_int
         L.pdf_lumi_events.argtypes = [_vp, _vp, ctypes.c_int, _ip, _ip, _dp, _ll, _vp, _vp, _vp, _vp, _vp, ctypes.c_int, _vp]
         L.pdf_xfxq2.restype = ctypes.c_int
@@ -140,11 +143,11 @@ def _check(rc: int, where: str):
         raise PdfbError(rc, where)
 
 
-def _dev_ptr(t, n, name):
-    """Pointer of a contiguous float64 CUDA tensor with at least n elements."""
+def _dev_ptr(t, n, name, dtype="float64"):
+    """Pointer of a contiguous CUDA tensor of the given dtype with at least n elements."""
     import torch
-    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
-        raise TypeError(f"{name} must be a contiguous float64 CUDA tensor")
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == getattr(torch, dtype) and t.is_contiguous()):
+        raise TypeError(f"{name} must be a contiguous {dtype} CUDA tensor")
     if t.numel() < n:
         raise ValueError(f"{name} has {t.numel()} elements, need {n}")
     return ctypes.c_void_p(t.data_ptr())
@@ -237,6 +240,24 @@ def pdf_lumi_events(g, terms, x1, x2, q2, lumi, alphas=None, alphas_out=None, di
                                _dev_ptr(alphas_out, n, "alphas_out") if alphas_out is not None else None,
                                1 if divide_by_x else 0, _stream_ptr(stream))
     _check(rc, "pdf_lumi_events")
+
+
+def pdf_xfxq2_pm(g, pids, x, q2, out, stream=None, n=None):
+    """pdf_xfxq2 with point-major output: out[n, n_req] (fp64)."""
+    pids = _i32(pids)
+    n = int(x.numel() if n is None else n)
+    rc = lib().pdf_xfxq2_pm(_vp(g), len(pids), pids.ctypes.data_as(_ip), n, _dev_ptr(x, n, "x"),
+                            _dev_ptr(q2, n, "q2"), _dev_ptr(out, len(pids) * n, "out"), _stream_ptr(stream))
+    _check(rc, "pdf_xfxq2_pm")
+
+
+def pdf_xfxq2_f32(g, pids, x, q2, out, stream=None, n=None):
+    """pdf_xfxq2 with fp32 output (fp64 arithmetic, one rounding at the store): out[n_req, n] float32."""
+    pids = _i32(pids)
+    n = int(x.numel() if n is None else n)
+    rc = lib().pdf_xfxq2_f32(_vp(g), len(pids), pids.ctypes.data_as(_ip), n, _dev_ptr(x, n, "x"),
+                             _dev_ptr(q2, n, "q2"), _dev_ptr(out, len(pids) * n, "out", dtype="float32"), _stream_ptr(stream))
+    _check(rc, "pdf_xfxq2_f32")
 
 
 def pdf_xfxq(g, pids, x, q, out, stream=None, n=None):

@@ -312,6 +312,32 @@ extern "C" int pdf_xfxq2(const pdfb_grid *g, int n_req, const int *pids, long lo
     return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, out, n, (cudaStream_t)cuda_stream);
 }
 
+// the two layout / precision variants of pdf_xfxq2 (compile-time kernel variants)
+static int xfxq2_variant(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x, const double *q2,
+                         void *out, void *cuda_stream, int mode)
+{
+    if (!g || !pids || n < 0) return PDFB_EINVAL;
+    if (n > 0 && (!x || !q2 || !out)) return PDFB_EINVAL;
+    int cols[PDFB_MAX_PIDS];
+    int rc = resolve_cols(g, n_req, pids, cols);
+    if (rc) return rc;
+    DeviceGuard guard(g->device);
+    if (!guard.ok) return PDFB_ECUDA;
+    return pdfb_launch_xfxq2(g, n_req, cols, n, x, q2, (double *)out, n, (cudaStream_t)cuda_stream, mode);
+}
+
+extern "C" int pdf_xfxq2_pm(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                            const double *q2, double *out, void *cuda_stream)
+{
+    return xfxq2_variant(g, n_req, pids, n, x, q2, out, cuda_stream, 1 << 1);
+}
+
+extern "C" int pdf_xfxq2_f32(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
+                             const double *q2, float *out, void *cuda_stream)
+{
+    return xfxq2_variant(g, n_req, pids, n, x, q2, out, cuda_stream, 2 << 1);
+}
+
 extern "C" int pdf_xfxq(const pdfb_grid *g, int n_req, const int *pids, long long n, const double *x,
                         const double *q, double *out, void *cuda_stream)
 {

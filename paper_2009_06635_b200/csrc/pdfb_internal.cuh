@@ -264,9 +264,10 @@ void pdfb_fill_lut(unsigned short *lut, const double *Z, const double *R, int nk
 void pdfb_count_launch(int n);
 
 // kernels' host launchers
-// q_is_q != 0: the scale array holds Q in GeV, not Q^2; the kernels square it once on load
+// mode = Q_IS_Q | OUT << 1 (xfxq2_smem.cuh): bit 0: the scale array holds Q in GeV, squared once on load;
+// OUT 0 / 1 / 2: fp64 flavour-major / fp64 point-major / fp32 flavour-major output
 int pdfb_launch_xfxq2(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                      const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q = 0,
+                      const double *q2, double *out, long long out_stride, cudaStream_t st, int mode = 0,
                       int member0 = 0, int n_mem = 1);
 int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, double *out,
                        cudaStream_t st, int q_is_q = 0);
@@ -277,7 +278,7 @@ int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off,
 int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_lumi_plan(pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int mode,
                            int member0, int n_mem);
 int pdfb_setup_ln(const double *d_raw, double *d_z, int n, cudaStream_t st);
 int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, const double *d_q2k, unsigned char *d_lines,

@@ -283,11 +283,12 @@ __device__ __noinline__ YW<W> slow_corner(const GridDev *gp, unsigned char *smem
 }
 
 // `count` entries of one class list of this warp (a multiple of 32 except at the very end), 32 at a time.
-template <bool Q_IS_Q, int W>
+template <int MODE, int W>
 __device__ __noinline__ void flush_class(int cls, int count, const uint32_t *list, const GridDev *gp, unsigned char *smem,
                                          const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
-                                         long long out_stride, const int *rowp)
+                                         long long out_stride, int n_req, const int *rowp)
 {
+    constexpr bool Q_IS_Q = MODE & 1;
     const int lane = threadIdx.x & 31, lane8 = threadIdx.x & 7;
     const int row[4] = {rowp[0], rowp[1], rowp[2], rowp[3]};
     for (int e = lane; e < count; e += 32) {
@@ -301,15 +302,15 @@ __device__ __noinline__ void flush_class(int cls, int count, const uint32_t *lis
         case 3: r = slow_corner<W, true>(gp, smem, xv, qv); break;
         default: r = slow_corner<W, false>(gp, smem, xv, qv); break;
         }
-        store_cols<W>(out, out_stride, p, row, r.v);
+        store_cols<W, (MODE >> 1)>(out, out_stride, n_req, p, row, r.v);
     }
 }
 
 // The full batches (final: all entries) of this warp's class lists; a remainder moves to the front.
-template <bool Q_IS_Q, int W>
+template <int MODE, int W>
 __device__ __noinline__ void flush_warp_lists(bool final, uint32_t *wl, unsigned char *cnt, unsigned char *req, const GridDev *gp,
                                               unsigned char *smem, const double *__restrict__ x, const double *__restrict__ q2,
-                                              double *__restrict__ out, long long out_stride, const int *rowp)
+                                              double *__restrict__ out, long long out_stride, int n_req, const int *rowp)
 {
     const int lane = threadIdx.x & 31;
     __syncwarp();
@@ -320,7 +321,7 @@ __device__ __noinline__ void flush_warp_lists(bool final, uint32_t *wl, unsigned
         const int take = final ? n : (n & ~31);
         if (take == 0) continue;
         uint32_t *list = wl + c * PDFB_SLOW_LCAP;
-        flush_class<Q_IS_Q, W>(c, take, list, gp, smem, x, q2, out, out_stride, rowp);
+        flush_class<MODE, W>(c, take, list, gp, smem, x, q2, out, out_stride, n_req, rowp);
         const int rem = n - take;  // < 32: moved to the front of the list
         uint32_t keep = 0;
         if (lane < rem) keep = __ldcg(list + take + lane);

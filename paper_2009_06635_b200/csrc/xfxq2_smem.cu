@@ -28,12 +28,14 @@
 
 #include "xfxq2_slow.cuh"
 
-template <bool Q_IS_Q, int W>  // compile-time: a run-time flag costs 11 % (register pressure at the 128 cap)
+template <int MODE, int W>  // compile-time (xfxq2_smem.cuh): a run-time flag costs 11 % (register pressure at the 128 cap)
 __global__ void __launch_bounds__(NT_SMEM, 1)
 k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
              const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
              long long out_stride, int member0, int n_req, int n_jobs)
 {
+    constexpr bool Q_IS_Q = MODE & 1;
+    constexpr int OUT = MODE >> 1;
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) unsigned long long mbar;
     __shared__ unsigned char wcnt[NT_SMEM / 32][8];  // entries in each warp's class lists
@@ -42,7 +44,9 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     // job = (member of the set, pass): blockIdx.x = seq * n_jobs + job; a job's CTAs share its tiles
     const int job = blockIdx.x % n_jobs, seq = blockIdx.x / n_jobs, nseq = gridDim.x / n_jobs;
     const int pass = job % pl.n, mem = job / pl.n;
-    out += (long long)mem * n_req * out_stride;
+    // (the members of a set follow each other in `out`; fp32 output counts in floats)
+    out = (OUT == PDFB_OUT_FM32) ? reinterpret_cast<double *>(reinterpret_cast<float *>(out) + (long long)mem * n_req * out_stride)
+                                 : out + (long long)mem * n_req * out_stride;
     const uint32_t tab = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)g.pre_bytes;
     const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&mbar);
     const int slice_bytes = (W == 4) ? g.slice_bytes : g.slice2_bytes;
@@ -103,7 +107,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     };
     constexpr int TILE = NT_SMEM * PPT_SMEM;
     auto flush_lists = [&](bool final) {  // warp-uniform
-        flush_warp_lists<Q_IS_Q, W>(final, wlist(), &wcnt[threadIdx.x >> 5][0], &s_req[threadIdx.x >> 5], &g, smem, x, q2, out, out_stride, pl.row[pass]);
+        flush_warp_lists<MODE, W>(final, wlist(), &wcnt[threadIdx.x >> 5][0], &s_req[threadIdx.x >> 5], &g, smem, x, q2, out, out_stride, n_req, pl.row[pass]);
     };
 
     bool pending = false;  // this warp has list entries (the flush request is only looked at then)
@@ -151,7 +155,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                 } else {
                     eval_stencil<W>(tab, RB, rb2, rb3, gi - 1, i - 1, wu, vw, lane8, y);
                 }
-                if (in_range[k]) store_cols<W>(out, out_stride, p0 + k * NT_SMEM, row, y);
+                if (in_range[k]) store_cols<W, OUT>(out, out_stride, n_req, p0 + k * NT_SMEM, row, y);
             }
         }
 #pragma unroll
@@ -164,7 +168,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                 double nanv[W];
 #pragma unroll
                 for (int c = 0; c < W; c++) nanv[c] = qnan;
-                store_cols<W>(out, out_stride, p, row, nanv);
+                store_cols<W, OUT>(out, out_stride, n_req, p, row, nanv);
                 if (job == 0) atomicAdd(g.n_invalid, 1ULL);
             }
             const unsigned slow_mask = __ballot_sync(0xffffffffu, slow);
@@ -222,10 +226,12 @@ int pdfb_smem_eligible(const pdfb_grid *g)
     const unsigned long long bit = 1ULL << (g->device & 63);
     if (!(attr_done.load(std::memory_order_acquire) & bit)) {
         const int lim = dev_max - STATIC_SMEM;
-        if (cudaFuncSetAttribute(k_xfxq2_smem<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfxq2_smem<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfxq2_smem<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess ||
-            cudaFuncSetAttribute(k_xfxq2_smem<true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim) != cudaSuccess) {
+        cudaError_t e = cudaSuccess;
+#define PDFB_ATTR(M, WW) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_xfxq2_smem<M, WW>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim)
+        PDFB_ATTR(0, 4); PDFB_ATTR(1, 4); PDFB_ATTR(2, 4); PDFB_ATTR(4, 4);
+        PDFB_ATTR(0, 2); PDFB_ATTR(1, 2); PDFB_ATTR(2, 2); PDFB_ATTR(4, 2);
+#undef PDFB_ATTR
+        if (e != cudaSuccess) {
             cudaGetLastError();
             return 0;
         }
@@ -233,7 +239,7 @@ int pdfb_smem_eligible(const pdfb_grid *g)
     }
     // the scratch-slot invariant, checked rather than assumed: one resident CTA per SM
     int occ = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfxq2_smem<false, 4>, NT_SMEM, PDFB_SMEM_FLOOR) != cudaSuccess || occ != 1) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_xfxq2_smem<0, 4>, NT_SMEM, PDFB_SMEM_FLOOR) != cudaSuccess || occ != 1) {
         cudaGetLastError();
         return 0;
     }
@@ -263,7 +269,7 @@ static int build_passes(int W, int n_groups, int n_req, const int *cols, PassLis
 }
 
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
-                           const double *q2, double *out, long long out_stride, cudaStream_t st, int q_is_q,
+                           const double *q2, double *out, long long out_stride, cudaStream_t st, int mode,
                            int member0, int n_mem)
 {
     // Width: a 4-column pass costs ~5.6 shared-memory wavefronts per point (4 gather + 1.6 setup and
@@ -294,9 +300,12 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
         const long long tiles = (m + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
         if (per_job > tiles) per_job = (int)tiles;
         const unsigned grid = (unsigned)(per_job * n_jobs);
-#define PDFB_LAUNCH(Q, WW) k_xfxq2_smem<Q, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, m, x + off, q2 + off, out + off, out_stride, member0, n_req, (int)n_jobs)
-        if (W == 4) { if (q_is_q) PDFB_LAUNCH(true, 4); else PDFB_LAUNCH(false, 4); }
-        else        { if (q_is_q) PDFB_LAUNCH(true, 2); else PDFB_LAUNCH(false, 2); }
+#define PDFB_LAUNCH(M, WW) k_xfxq2_smem<M, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, m, x + off, q2 + off, out_off, out_stride, member0, n_req, (int)n_jobs)
+        // element offset of this slice in `out` (doubles, or floats for the fp32 variant)
+        const long long eo = (mode >> 1) == PDFB_OUT_PM64 ? off * n_req : off;
+        double *out_off = (mode >> 1) == PDFB_OUT_FM32 ? reinterpret_cast<double *>(reinterpret_cast<float *>(out) + eo) : out + eo;
+        if (W == 4) { if (mode == 0) PDFB_LAUNCH(0, 4); else if (mode == 1) PDFB_LAUNCH(1, 4); else if (mode == 2) PDFB_LAUNCH(2, 4); else PDFB_LAUNCH(4, 4); }
+        else        { if (mode == 0) PDFB_LAUNCH(0, 2); else if (mode == 1) PDFB_LAUNCH(1, 2); else if (mode == 2) PDFB_LAUNCH(2, 2); else PDFB_LAUNCH(4, 2); }
 #undef PDFB_LAUNCH
         pdfb_count_launch(1);
     }

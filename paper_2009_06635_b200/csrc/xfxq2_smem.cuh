@@ -221,21 +221,33 @@ __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, d
 
 template <int W> struct YW { double v[W]; };  // one point's W columns, in column order
 
+// Kernel variants (compile-time): MODE = Q_IS_Q | OUT << 1.
+//   Q_IS_Q  the scale array holds Q in GeV (pdf_xfxq), squared once on load
+//   OUT     0: fp64, flavour-major out[r * stride + p]              (pdf_xfxq2, the contract layout)
+//           1: fp64, point-major   out[p * n_req + r]               (pdf_xfxq2_pm)
+//           2: fp32, flavour-major ((float *)out)[r * stride + p]   (pdf_xfxq2_f32: fp64 arithmetic, one rounding at the store)
+#define PDFB_OUT_FM64 0
+#define PDFB_OUT_PM64 1
+#define PDFB_OUT_FM32 2
+
+template <int OUT>
+__device__ __forceinline__ void store_one(double *__restrict__ out, long long out_stride, int n_req, long long p, int r, double v)
+{
+    if (OUT == PDFB_OUT_FM64) __stcs(out + r * out_stride + p, v);
+    else if (OUT == PDFB_OUT_PM64) __stcs(out + p * n_req + r, v);
+    else __stcs(reinterpret_cast<float *>(out) + r * out_stride + p, (float)v);
+}
+
 // one point's W columns to their output rows (row < 0: column not requested)
-template <int W>
-__device__ __forceinline__ void store_cols(double *__restrict__ out, long long out_stride, long long p,
+template <int W, int OUT>
+__device__ __forceinline__ void store_cols(double *__restrict__ out, long long out_stride, int n_req, long long p,
                                            const int row[W], const double v[W])
 {
-#ifdef PDFB_STORE_DEFAULT
-#define PDFB_ST(ptr, val) (*(ptr) = (val))
-#else
-#define PDFB_ST(ptr, val) __stcs(ptr, val)
-#endif
-    if (row[0] >= 0) PDFB_ST(out + row[0] * out_stride + p, v[0]);
-    if (row[1] >= 0) PDFB_ST(out + row[1] * out_stride + p, v[1]);
+    if (row[0] >= 0) store_one<OUT>(out, out_stride, n_req, p, row[0], v[0]);
+    if (row[1] >= 0) store_one<OUT>(out, out_stride, n_req, p, row[1], v[1]);
     if (W == 4) {
-        if (row[W - 2] >= 0) PDFB_ST(out + row[W - 2] * out_stride + p, v[W - 2]);
-        if (row[W - 1] >= 0) PDFB_ST(out + row[W - 1] * out_stride + p, v[W - 1]);
+        if (row[W - 2] >= 0) store_one<OUT>(out, out_stride, n_req, p, row[W - 2], v[W - 2]);
+        if (row[W - 1] >= 0) store_one<OUT>(out, out_stride, n_req, p, row[W - 1], v[W - 1]);
     }
 }
 

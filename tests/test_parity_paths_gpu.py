@@ -171,3 +171,41 @@ def test_rule_C_small_y0_branch(torch_cuda, monkeypatch, force_fallback):
     st = check_parity(out.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what=f"rule C small y0, fallback={force_fallback}")
     print(st)
     B.pdf_grid_free(h)
+
+
+@pytest.mark.parametrize("force_fallback", [False, True])
+def test_point_major_and_fp32_output(torch_cuda, grid2, ograph2, monkeypatch, force_fallback):
+    """pdf_xfxq2_pm / pdf_xfxq2_f32: compile-time variants of the same
+    kernels.  Point-major: bit-identical to pdf_xfxq2 transposed.  fp32: the fp64 result of pdf_xfxq2
+    rounded once (bit-identical to casting it), hence within half an fp32 ulp + the fp64 tolerance of
+    the oracle.  The extrapolation mix (class lists), the scan, PID subsets over 1-3 groups and the
+    2-column plan; both kernels."""
+    torch = torch_cuda
+    if force_fallback:
+        monkeypatch.setenv("PDFB_FORCE_FALLBACK", "1")
+    h = B.load_pdf_spec(grid2)
+    monkeypatch.delenv("PDFB_FORCE_FALLBACK", raising=False)
+    assert bool(B.pdf_grid_uses_smem_path(h)) != force_fallback
+    x, q2 = W.queries_extrapolation_mix(grid2, 120_011)
+    xs, qs = W.scan_points(grid2, per_cell=1)
+    x, q2 = np.concatenate([x, xs, [0.5, -1.0, 2.0]]), np.concatenate([q2, qs, [np.nan, 10.0, 10.0]])
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    n = len(x)
+    for req in (list(W.PIDS_11), [21], [3, -5, 0, 3, 1]):
+        fm = torch.empty((len(req), n), dtype=torch.float64, device="cuda")
+        pm = torch.full((n, len(req)), 7.0, dtype=torch.float64, device="cuda")
+        f32 = torch.full((len(req), n), 7.0, dtype=torch.float32, device="cuda")
+        B.pdf_xfxq2(h, req, dx, dq, fm)
+        B.pdf_xfxq2_pm(h, req, dx, dq, pm)
+        B.pdf_xfxq2_f32(h, req, dx, dq, f32)
+        torch.cuda.synchronize()
+        assert torch.equal(torch.nan_to_num(pm.t().contiguous(), nan=-9.0), torch.nan_to_num(fm, nan=-9.0))
+        assert torch.equal(torch.nan_to_num(f32, nan=-9.0), torch.nan_to_num(fm.to(torch.float32), nan=-9.0))
+        ref, sc = ograph2.xfxq2(req, x, q2, with_scale=True)
+        check_parity(pm.t().cpu().numpy(), ref, sc, max_clause_frac=5e-3, what=f"point-major {req} fallback={force_fallback}")
+        got32 = f32.cpu().numpy().astype(np.float64)
+        ok = ~np.isnan(ref)
+        assert np.array_equal(np.isnan(got32), np.isnan(ref))
+        half_ulp32 = 0.5 * np.spacing(np.abs(ref[ok]).astype(np.float32)).astype(np.float64)
+        assert np.all(np.abs(got32[ok] - ref[ok]) <= half_ulp32 + 1e-12 * np.abs(ref[ok]) + 1e-15 + 1e-12 * sc[ok])
+    B.pdf_grid_free(h)
