@@ -40,6 +40,9 @@ enum {
     PDFB_ECUDA = -4,    /* CUDA runtime error (no device, out of memory, launch failure) */
     PDFB_EIO = -6,      /* a file could not be opened or read                          */
     PDFB_EFORMAT = -7,  /* a file is not in the expected text layout                   */
+    PDFB_EXKNOTS = -8,  /* a well-formed member file whose sub-grids carry different x-knot
+                           arrays (or PID lists): LHAPDF allows it, this library wants one
+                           x-knot array for all sub-grids (pdf_grid_load's argument list)  */
     PDFB_ELIMIT = -5    /* more than PDFB_MAX_SUBGRIDS subgrids or PDFB_MAX_PIDS PIDs    */
 };
 #define PDFB_MAX_SUBGRIDS 16
@@ -230,7 +233,9 @@ long long pdfb_launch_count(void);
  * Member file ("lhagrid1"): metadata header, then blocks separated by lines "---"; a block is the
  * x knots (line 1), the Q knots in GeV (line 2), the PIDs (line 3), then nx*nq lines of n_pid
  * values, x index outer, Q index inner -- pdf_grid_load's own order.  All blocks must share one
- * x-knot array and one PID list (else PDFB_EKNOTS).  PDFB_EIO: cannot read; PDFB_EFORMAT: not this
+ * x-knot array and one PID list: a file whose blocks differ there is read to the end, found
+ * well-formed, and refused with PDFB_EXKNOTS (distinct from PDFB_EKNOTS / PDFB_EFORMAT, so that a
+ * caller can tell "valid LHAPDF file this library cannot take" from "broken file").  PDFB_EIO: cannot read; PDFB_EFORMAT: not this
  * layout.  The handle owns host memory until pdfb_lhagrid_free.
  *   pdfb_lhagrid_get fills caller arrays sized from pdfb_lhagrid_dims:
  *   x_knots[nx], q_offsets[n_sub+1], q_knots[nq_tot], pids[n_pid], values[nx*nq_tot*n_pid].

@@ -26,7 +26,7 @@ EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_member
            "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
 
 
-PDFB_EINVAL, PDFB_EKNOTS, PDFB_EPID, PDFB_ECUDA, PDFB_ELIMIT, PDFB_EIO, PDFB_EFORMAT = -1, -2, -3, -4, -5, -6, -7
+PDFB_EINVAL, PDFB_EKNOTS, PDFB_EPID, PDFB_ECUDA, PDFB_ELIMIT, PDFB_EIO, PDFB_EFORMAT, PDFB_EXKNOTS = -1, -2, -3, -4, -5, -6, -7, -8
 
 
 class PdfbError(RuntimeError):

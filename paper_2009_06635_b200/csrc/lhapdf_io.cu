@@ -82,6 +82,7 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
     ++i;
     std::vector<double> row, xk, qk;
     int rc = PDFB_OK;
+    bool mixed_x = false;  // blocks with different x knots / PIDs: parsed to the end, then refused as such
     g->q_off.push_back(0);
     while (i < lines.size() && !rc) {
         while (i < lines.size() && is_blank(lines[i])) ++i;
@@ -96,14 +97,13 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
         if (g->n_sub == 0) {
             g->x = xk; g->nx = (int)xk.size(); g->pids = pids; g->n_pid = (int)pids.size();
         } else if (xk != g->x || pids != g->pids) {
-            rc = PDFB_EKNOTS;  // this library wants one x-knot array and one PID list for all sub-grids
-            break;
+            mixed_x = true;  // this library wants one x-knot array and one PID list for all sub-grids
         }
         const size_t nrows = xk.size() * qk.size();
         for (size_t r = 0; r < nrows && !rc; r++, i++) {
             if (i >= lines.size() || is_sep(lines[i]) || !parse_doubles(lines[i].first, lines[i].second, row) ||
-                row.size() != (size_t)g->n_pid) { rc = PDFB_EFORMAT; break; }
-            g->values.insert(g->values.end(), row.begin(), row.end());
+                row.size() != pids.size()) { rc = PDFB_EFORMAT; break; }
+            if (!mixed_x) g->values.insert(g->values.end(), row.begin(), row.end());
         }
         if (rc) break;
         g->q.insert(g->q.end(), qk.begin(), qk.end());
@@ -116,6 +116,7 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
         }
     }
     if (!rc && g->n_sub == 0) rc = PDFB_EFORMAT;
+    if (!rc && mixed_x) rc = PDFB_EXKNOTS;
     if (!rc && g->n_sub > PDFB_MAX_SUBGRIDS) rc = PDFB_ELIMIT;
     if (rc) { delete g; return rc; }
     *out = g;

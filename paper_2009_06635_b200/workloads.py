@@ -332,14 +332,24 @@ def scan_points(grid: PdfGridSpec, per_cell: int = 3):
 # Writers for the LHAPDF6 text layout (the files themselves are not available here: tests and
 # users write synthetic sets with these and read them back through the library's front-end)
 # --------------------------------------------------------------------------
-def write_lhagrid(spec: PdfGridSpec, path: str, pdf_type: str = "central") -> None:
+def write_lhagrid(spec: PdfGridSpec, path: str, pdf_type: str = "central", x_knots_per_sub=None) -> None:
+    """Member file in the LHAPDF6 text layout.  ``x_knots_per_sub`` (a list of x-knot arrays, one per
+    sub-grid) writes a file whose sub-grids carry DIFFERENT x knots -- legal in LHAPDF, refused by
+    this library with PDFB_EXKNOTS; the values of such a block are the analytic family of
+    ``spec.params`` on those knots (the file is for reader tests)."""
     r = lambda a: " ".join(repr(float(v)) for v in a)
     with open(path, "w") as f:
         f.write(f"PdfType: {pdf_type}\nFormat: lhagrid1\n---\n")
         for s in range(spec.n_sub):
             q = spec.sub_q(s)
-            f.write(r(spec.x_knots) + "\n" + r(q) + "\n" + " ".join(str(int(p)) for p in spec.pids) + "\n")
-            for row in spec.sub_values(s).reshape(spec.nx * len(q), spec.n_pid):
+            if x_knots_per_sub is None:
+                xk, vals = spec.x_knots, spec.sub_values(s).reshape(spec.nx * len(q), spec.n_pid)
+            else:
+                xk = np.asarray(x_knots_per_sub[s], dtype=np.float64)
+                vals = np.stack([family_value(spec.params[int(p)], xk[:, None], (q * q)[None, :]) for p in spec.pids], axis=-1)
+                vals = vals.reshape(len(xk) * len(q), spec.n_pid)
+            f.write(r(xk) + "\n" + r(q) + "\n" + " ".join(str(int(p)) for p in spec.pids) + "\n")
+            for row in vals:
                 f.write(r(row) + "\n")
             f.write("---\n")
 

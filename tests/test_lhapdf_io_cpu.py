@@ -81,4 +81,17 @@ def test_missing_file_and_mismatched_blocks(tmp_path):
     (tmp_path / "bad.dat").write_text("---\n".join(blocks))
     with pytest.raises(B.PdfbError) as e:
         B.lhagrid_read(str(tmp_path / "bad.dat"))
-    assert e.value.code == B.PDFB_EKNOTS
+    assert e.value.code == B.PDFB_EXKNOTS
+    # a complete, well-formed member file whose sub-grids have x-knot arrays of different LENGTHS (as
+    # LHAPDF allows): read to the end and refused with the distinct code, not as a malformed file
+    xs = [spec.x_knots, W._geomspace(1e-9, 1.0, 80), spec.x_knots[::2].copy(), W._geomspace(1e-9, 1.0, 120)]
+    W.write_lhagrid(spec, str(tmp_path / "perx.dat"), x_knots_per_sub=xs)
+    with pytest.raises(B.PdfbError) as e:
+        B.lhagrid_read(str(tmp_path / "perx.dat"))
+    assert e.value.code == B.PDFB_EXKNOTS and "x-knot" in str(e.value)
+    # ... while the same file cut short is still a malformed file
+    txt = (tmp_path / "perx.dat").read_text().split("\n")
+    (tmp_path / "perx_cut.dat").write_text("\n".join(txt[: len(txt) // 2]) + "\n")
+    with pytest.raises(B.PdfbError) as e:
+        B.lhagrid_read(str(tmp_path / "perx_cut.dat"))
+    assert e.value.code == B.PDFB_EFORMAT
