@@ -30,6 +30,7 @@ N_FULL = 100_000_000
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_xfxq2_smem launch at 1e8 points x 11
 # flavours, from the `ncu --set full` capture summarised in profiles/r1_xfxq2_smem_full.md
 NCU_TRAFFIC_BYTES_PER_POINT = (1.605477e9 + 8.741274e9) / 1e8
+NCU_TRAFFIC_SOURCE = "profiles/r1_xfxq2_smem_full.md (ncu, 1e8 points; scaled by points)"
 
 
 def measured_peaks():
@@ -88,9 +89,13 @@ class ClockSampler(threading.Thread):
 
 
 def cpu_baseline(grid, x, q2, pids, target_s=12.0):
-    """The oracle as it stands, on the first points of the same batch (bounded sample)."""
+    """The oracle as it stands, on the first points of the same batch (bounded sample): once with all
+    host cores (the reported value) and once with one thread.  The oracle takes its
+    coordinate logarithms in binary128 (reading R-ln): slower than a libm-log oracle
+    would be, and stated as such."""
     import oracle
     og = oracle.OraclePdfGrid.from_spec(grid)
+    cores = oracle.threads()
     m = min(len(x), 200_000)
     t = time.perf_counter()
     og.xfxq2(pids, x[:m], q2[:m])
@@ -99,8 +104,16 @@ def cpu_baseline(grid, x, q2, pids, target_s=12.0):
     t = time.perf_counter()
     og.xfxq2(pids, x[:m], q2[:m])
     dt = time.perf_counter() - t
-    return {"value": m * len(pids) / dt, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
-            "sample": f"first {m} points of the config-3 batch x {len(pids)} flavours, {dt:.1f} s"}
+    m1 = max(20_000, int(m / cores / 3))          # ~4 s on one thread
+    oracle.set_threads(1)
+    t = time.perf_counter()
+    og.xfxq2(pids, x[:m1], q2[:m1])
+    dt1 = time.perf_counter() - t
+    oracle.set_threads(cores)
+    return {"value": m * len(pids) / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {m} points of the config-3 batch x {len(pids)} flavours, {dt:.1f} s",
+            "value_1_thread": m1 * len(pids) / dt1, "sample_1_thread": f"first {m1} points, {dt1:.1f} s",
+            "note": "oracle ln = binary128 logq rounded once (reading R-ln): slower than a libm-log oracle"}
 
 
 def parity_population(torch, out_d, grid, x_h, q2_h, pids, chunk=10_000_000):
@@ -148,51 +161,105 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def bench_other_configs(torch, B, h, ha, grid, peak):
-    """Configs 1, 2, 4 and 5 of BASELINE.json at their full sizes, device-resident, reported beside
-    the metric (parity-test cases, not the headline): kernel time by CUDA events, 5 repetitions."""
-    def timed(fn, reps=5):
-        for _ in range(2):
-            fn()
-        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a.record()
-        for _ in range(reps):
-            fn()
-        b.record(); torch.cuda.synchronize()
-        return a.elapsed_time(b) / reps
+# Algorithmic FP64-pipe instruction counts per point, frozen in SURVEY.md 8(d) (FMA = 1):
+#   in range W(F) = 2*28 + 32 + 16 + 16 F;  rules A / B ~ 120 + 120 F;  rule C ~ 136 + 110 F
+def w_in(F):
+    return 2 * 28 + 32 + 16 + 16 * F
 
+
+def w_ab(F):
+    return 120 + 120 * F
+
+
+def w_c(F):
+    return 136 + 110 * F
+
+
+def w_config4(F):
+    """Mix of reading Q14: 70 % in range, 20 % rule A, 5 % Q above / 5 % Q below the grid with x
+    log-uniform on [1e-12, 1], i.e. a quarter of each in the corner (the Q^2 rule on two rule-A values)."""
+    return 0.70 * w_in(F) + 0.20 * w_ab(F) + 0.0375 * w_ab(F) + 0.0125 * 2 * w_ab(F) + 0.0375 * w_c(F) + 0.0125 * (w_c(F) + w_ab(F))
+
+
+def roofline_entry(ms, n_points, bytes_per_point, w_per_point, hbm_gbs, fma_per_s):
+    """Fractions of the two contract bounds and of the slower one (north_star: "the roofline is the
+    slower of two bounds")."""
+    t = ms * 1e-3
+    t_hbm, t_fp64 = bytes_per_point * n_points / (hbm_gbs * 1e9), w_per_point * n_points / fma_per_s
+    return {"hbm_frac": t_hbm / t, "fp64_frac": t_fp64 / t, "bound": "hbm" if t_hbm >= t_fp64 else "fp64",
+            "roofline_ms": max(t_hbm, t_fp64) * 1e3, "roofline_frac": max(t_hbm, t_fp64) / t,
+            "fp64_ops_per_point": w_per_point, "bytes_per_point": bytes_per_point}
+
+
+def timed_reps(torch, fn, reps=20, warm=3):
+    """Median and best of `reps` CUDA-event timings of fn() on the current stream."""
+    for _ in range(warm):
+        fn()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for a, b in ev:
+        a.record(); fn(); b.record()
+    torch.cuda.synchronize()
+    ts = sorted(a.elapsed_time(b) for a, b in ev)
+    return {"ms": float(np.median(ts)), "ms_best": ts[0], "reps": reps}
+
+
+def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s):
+    """Configs 1, 2, 4 and 5 of BASELINE.json at their full sizes, device-resident, reported beside
+    the metric (parity-test cases, not the headline): median and best of 20 CUDA-event timings, each
+    with its fraction of the slower contract bound."""
     def dev(*arrs):
         return [torch.from_numpy(a).cuda() for a in arrs]
+
+    def entry(t, n_points, F, bpp, w, **extra):
+        e = dict(t)
+        e["evaluations_per_s"] = n_points * F / (t["ms"] * 1e-3)
+        e.update(roofline_entry(t["ms"], n_points, bpp, w, peak, fma_per_s))
+        e.update(extra)
+        return e
 
     res, p11 = {}, list(W.PIDS_11)
     g1 = W.grid_config1()
     h1 = B.load_pdf_spec(g1)
     x, q2 = dev(*W.queries_in_range(g1, 10_000, 1))
     o = torch.empty((3, 10_000), dtype=torch.float64, device="cuda")
-    ms = timed(lambda: B.pdf_xfxq2(h1, list(W.PIDS_3), x, q2, o))
-    res["config1_1e4x3"] = {"ms": ms, "evaluations_per_s": 3e4 / (ms * 1e-3), "note": "launch-latency sized"}
+    res["config1_1e4x3"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2(h1, list(W.PIDS_3), x, q2, o)), 10_000, 3, 40, w_in(3),
+                                 note="launch-latency sized")
     B.pdf_grid_free(h1)
     x, q2 = dev(*W.queries_in_range(grid, 1_000_000, 2))
     o = torch.empty((11, 1_000_000), dtype=torch.float64, device="cuda")
-    ms = timed(lambda: B.pdf_xfxq2(h, p11, x, q2, o))
-    res["config2_1e6x11"] = {"ms": ms, "evaluations_per_s": 1.1e7 / (ms * 1e-3), "hbm_frac": 104e6 / (ms * 1e-3) / 1e9 / peak}
+    res["config2_1e6x11"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2(h, p11, x, q2, o)), 1_000_000, 11, 104, w_in(11))
     n4 = 10_000_000
     x, q2 = dev(*W.queries_extrapolation_mix(grid, n4))
     o = torch.empty((11, n4), dtype=torch.float64, device="cuda")
-    ms = timed(lambda: B.pdf_xfxq2(h, p11, x, q2, o))
-    res["config4_mix_1e7x11"] = {"ms": ms, "evaluations_per_s": 11 * n4 / (ms * 1e-3), "hbm_frac": 104 * n4 / (ms * 1e-3) / 1e9 / peak}
-    ms = timed(lambda: B.pdf_xfxq2(h, [21], x, q2, o))
-    res["config4_mix_1e7x1"] = {"ms": ms, "evaluations_per_s": n4 / (ms * 1e-3), "hbm_frac": 24 * n4 / (ms * 1e-3) / 1e9 / peak}
+    res["config4_mix_1e7x11"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2(h, p11, x, q2, o)), n4, 11, 104, w_config4(11))
+    res["config4_mix_1e7x1"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2(h, [21], x, q2, o)), n4, 1, 24, w_config4(1))
+    # the two output variants of SURVEY.md 8(f).4 on the same batch
+    opm = torch.empty((n4, 11), dtype=torch.float64, device="cuda")
+    o32 = torch.empty((11, n4), dtype=torch.float32, device="cuda")
+    res["config4_mix_1e7x11_point_major"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2_pm(h, p11, x, q2, opm), reps=10), n4, 11, 104, w_config4(11))
+    res["config4_mix_1e7x11_fp32_out"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2_f32(h, p11, x, q2, o32), reps=10), n4, 11, 60, w_config4(11))
+    del opm, o32
     x1, x2, q2 = dev(*W.queries_mc_events(grid, n4))
     o2 = torch.empty((11, n4), dtype=torch.float64, device="cuda")
     oa = torch.empty(n4, dtype=torch.float64, device="cuda")
 
     def events():
         B.pdf_xfxq2(h, p11, x1, q2, o); B.pdf_xfxq2(h, p11, x2, q2, o2); B.alphas_q2(ha, q2, oa)
-    ms = timed(events)
-    res["config5_1e7_events"] = {"ms": ms, "evaluations_per_s": 22 * n4 / (ms * 1e-3), "events_per_s": n4 / (ms * 1e-3),
-                                 "hbm_frac": (2 * 104 + 16) * n4 / (ms * 1e-3) / 1e9 / peak,
-                                 "calls": "pdf_xfxq2(x1), pdf_xfxq2(x2), alphas_q2 on the shared Q^2"}
+    t = timed_reps(torch, events)
+    res["config5_1e7_events"] = entry(t, 2 * n4, 11, 104 + 8, w_in(11) + 24, events_per_s=n4 / (t["ms"] * 1e-3),
+                                      calls="pdf_xfxq2(x1), pdf_xfxq2(x2), alphas_q2 on the shared Q^2 (per PDF point: 104 B + half of alpha_s' 16 B)")
+    # the fused call (luminosity sum over 11 flavour pairs + alpha_s), one number per event out
+    terms = [(q, -q, 1.0) for q in (1, 2, 3, 4, 5)] + [(-q, q, 1.0) for q in (1, 2, 3, 4, 5)] + [(21, 21, 0.25)]
+    lum = torch.empty(n4, dtype=torch.float64, device="cuda")
+    t = timed_reps(torch, lambda: B.pdf_lumi_events(h, terms, x1, x2, q2, lum, alphas=ha, alphas_out=oa))
+    w_ev = 3 * 28 + 3 * 16 + 2 * (16 + 16 * 11) + 2 * 11 * 11 + 48   # 3 ln, 3 weight sets, 2 x (outer product + contraction), bilinear form, alpha_s
+    e = dict(t)
+    e.update(roofline_entry(t["ms"], n4, 24 + 16, w_ev, peak, fma_per_s))
+    e.update({"events_per_s": n4 / (t["ms"] * 1e-3), "evaluations_per_s": 22 * n4 / (t["ms"] * 1e-3),
+              "speedup_vs_three_launches": res["config5_1e7_events"]["ms"] / t["ms"],
+              "calls": "pdf_lumi_events(x1, x2, Q^2) with alpha_s: 40 B per event of HBM traffic instead of 240 + 176 + the consumer's 176",
+              "onchip_gather_bound_ms": 2 * 16 * 12 * 8 * n4 / (128 * 148 * 1.965e9) * 1e3})
+    res["config5_fused_lumi"] = e
     return res
 
 
@@ -278,18 +345,21 @@ def run_gpu(args):
     launches = B.launch_count() - launches0
     clocks = sampler.stop()
     total_ms = t0.elapsed_time(t1)
-    kern_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+    per_step = sorted(a.elapsed_time(b) for a, b in evs)
+    kern_ms, kern_med, kern_best = float(np.mean(per_step)), float(np.median(per_step)), per_step[0]
     if dist is not None:
-        t = torch.tensor([total_ms, kern_ms], device="cuda", dtype=torch.float64)
+        t = torch.tensor([total_ms, kern_ms, kern_med, kern_best], device="cuda", dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, kern_ms = float(t[0]), float(t[1])
+        total_ms, kern_ms, kern_med, kern_best = (float(v) for v in t)
     ms_per_step = total_ms / args.steps
     value = world * n * F / (ms_per_step * 1e-3)
 
-    # ---- end to end: pinned host buffers through pdf_xfxq2_host, copies inside the timed region
+    # ---- end to end: pinned host buffers through pdf_xfxq2_host, copies inside the timed region.
+    # Every rank takes part (the value is the whole job's); the pinned buffers of all ranks together
+    # stay at one config-3 batch (10.4 GB), whatever the rank count.
     e2e = None
     if not args.no_e2e:
-        n_e = min(n, args.e2e_points)
+        n_e = min(n, max(1, args.e2e_points // world))
         xp = torch.from_numpy(x_h[:n_e]).pin_memory(); qp = torch.from_numpy(q2_h[:n_e]).pin_memory()
         op = torch.empty((F, n_e), dtype=torch.float64).pin_memory()
         B.pdf_xfxq2_host(h, pids, xp, qp, op)
@@ -304,8 +374,8 @@ def run_gpu(args):
             t = torch.tensor([e_s], device="cuda", dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             e_s = float(t[0])
-        e2e = {"value": world * n_e * F / e_s, "unit": UNIT, "h2d_bytes_per_step": 16 * n_e,
-               "d2h_bytes_per_step": 8 * F * n_e, "points_per_step": n_e, "ms_per_step": e_s * 1e3,
+        e2e = {"value": world * n_e * F / e_s, "unit": UNIT, "h2d_bytes_per_step": 16 * n_e * world,
+               "d2h_bytes_per_step": 8 * F * n_e * world, "points_per_step": n_e * world, "ms_per_step": e_s * 1e3,
                "api": "pdf_xfxq2_host (pinned host buffers, 3-stage copy/compute pipeline)"}
         del xp, qp, op
 
@@ -318,18 +388,15 @@ def run_gpu(args):
     aspec = W.make_alphas_grid()
     ha = B.load_alphas_spec(aspec, device=local)
     a_out = torch.empty(n, dtype=torch.float64, device="cuda")
-    for _ in range(3):
-        B.alphas_q2(ha, q2_d, a_out)
-    a0 = torch.cuda.Event(enable_timing=True); a1 = torch.cuda.Event(enable_timing=True)
-    a0.record()
-    for _ in range(5):
-        B.alphas_q2(ha, q2_d, a_out)
-    a1.record(); torch.cuda.synchronize()
-    a_ms = a0.elapsed_time(a1) / 5
+    a_t = timed_reps(torch, lambda: B.alphas_q2(ha, q2_d, a_out))
     peak, peak_src = measured_peaks()
     sms = torch.cuda.get_device_properties(local).multi_processor_count
+    # measured denominators for the two bounds MEASURED_PEAKS.json does not carry (pdfb_probe)
+    lds_bps, fma_ps = B.probe(B.PROBE_LDS, local), B.probe(B.PROBE_FP64, local)
     bytes_per_launch = (16 + 8 * F) * n
     achieved = bytes_per_launch / (kern_ms * 1e-3) / 1e9
+    w_f = w_in(F)
+    t_hbm, t_fp64, t_gather = bytes_per_launch / (peak * 1e9), w_f * n / fma_ps, 128.0 * F * n / lds_bps
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -341,29 +408,31 @@ def run_gpu(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": (NCU_TRAFFIC_BYTES_PER_POINT * n / 1e9) if F == 11 else None, "traffic_unit": "GB per launch",
-                         "traffic_source": "profiles/r1_xfxq2_smem_full.md (ncu, 1e8 points; scaled by points)",
+                         "traffic_source": NCU_TRAFFIC_SOURCE,
                          "kernel": "k_xfxq2_smem" if B.pdf_grid_uses_smem_path(h) else "k_xfxq2_v0", "kernel_ms": kern_ms,
-                         "algorithmic_bytes_per_point": 16 + 8 * F, "peak_source": peak_src},
-            # the limit the kernel actually runs against: the per-point 4x4 stencil gather,
-            # 16 x 8 B x F of table per point through the SM's 128 B/clk shared-memory data pipe
-            "onchip_gather": {"bound": "smem", "achieved": 128 * F * n / (kern_ms * 1e-3) / 1e9,
-                              "peak": sms * 128 * (clocks["sm_mhz"] or 1965.0) * 1e6 / 1e9, "unit": "GB/s",
-                              "algorithmic_bytes_per_point": 128 * F,
+                         "kernel_ms_median": kern_med, "kernel_ms_best": kern_best,
+                         "algorithmic_bytes_per_point": 16 + 8 * F, "peak_source": peak_src,
+                         # the same launch against the other contract bound and against the bound the design
+                         # actually runs into: every gathered table byte crosses the SM's
+                         # 128 B/clk shared-memory pipe, 16 x 8 B x F per point, measured peak (pdfb_probe)
+                         "fp64_frac": t_fp64 / (kern_ms * 1e-3), "slower_contract_bound": "hbm" if t_hbm >= t_fp64 else "fp64",
+                         "bound_onchip_ms": t_gather * 1e3, "bound_onchip_frac": t_gather / (kern_ms * 1e-3),
+                         "bound_onchip_as_roofline_frac": max(t_hbm, t_fp64) / t_gather,
+                         "bound_onchip_note": "a per-point gather cannot run faster than bound_onchip_ms: at most "
+                                              "bound_onchip_as_roofline_frac of the contract roofline (DESIGN.md 6)"},
+            "onchip_gather": {"bound": "smem", "achieved": 128 * F * n / (kern_ms * 1e-3) / 1e9, "peak": lds_bps / 1e9,
+                              "peak_nominal": sms * 128 * (clocks["sm_mhz"] or 1965.0) * 1e6 / 1e9, "unit": "GB/s",
+                              "frac": t_gather / (kern_ms * 1e-3), "algorithmic_bytes_per_point": 128 * F,
+                              "peak_source": "measured: pdfb_probe(PDFB_PROBE_LDS), conflict-free LDS.128",
                               "note": "context only; the contract roofline is `roofline` (HBM)"},
-            "alphas": {"points": n, "ms": a_ms, "evaluations_per_s": n / (a_ms * 1e-3),
-                       "hbm_frac": 16 * n / (a_ms * 1e-3) / 1e9 / peak}}
-    # measured denominators for the two bounds MEASURED_PEAKS.json does not carry (pdfb_probe)
-    lds_bps, fma_ps = B.probe(B.PROBE_LDS, local), B.probe(B.PROBE_FP64, local)
-    og = line["onchip_gather"]
-    og["peak_nominal"], og["peak"], og["peak_source"] = og["peak"], lds_bps / 1e9, "measured: pdfb_probe(PDFB_PROBE_LDS), conflict-free LDS.128"
-    og["frac"] = og["achieved"] / og["peak"]
-    w_f = 2 * 28 + 32 + 16 + 16 * F  # algorithmic FP64-pipe operations per in-range point, SURVEY.md 8(d)
-    line["fp64"] = {"bound": "alu", "achieved": w_f * n / (kern_ms * 1e-3) / 1e12, "peak": fma_ps / 1e12,
-                    "unit": "T FP64 op/s (FMA = 1)", "frac": w_f * n / (kern_ms * 1e-3) / fma_ps,
-                    "algorithmic_ops_per_point": w_f, "peak_source": "measured: pdfb_probe(PDFB_PROBE_FP64), DFMA chains",
-                    "note": "context only; HBM is the slower of the two contract bounds"}
+            "fp64": {"bound": "alu", "achieved": w_f * n / (kern_ms * 1e-3) / 1e12, "peak": fma_ps / 1e12,
+                     "unit": "T FP64 op/s (FMA = 1)", "frac": t_fp64 / (kern_ms * 1e-3),
+                     "algorithmic_ops_per_point": w_f, "peak_source": "measured: pdfb_probe(PDFB_PROBE_FP64), DFMA chains",
+                     "note": "context only; HBM is the slower of the two contract bounds"},
+            "alphas": {"points": n, "ms": a_t["ms"], "ms_best": a_t["ms_best"], "evaluations_per_s": n / (a_t["ms"] * 1e-3),
+                       **roofline_entry(a_t["ms"], n, 16, 48, peak, fma_ps)}}
     if not args.no_other_configs:
-        line["other_configs"] = bench_other_configs(torch, B, h, ha, grid, peak)
+        line["other_configs"] = bench_other_configs(torch, B, h, ha, grid, peak, fma_ps)
     B.alphas_grid_free(ha)
     if not args.no_members:
         line["multi_member"] = bench_members(torch, B, local, args.members)
@@ -379,14 +448,26 @@ def run_gpu(args):
     print(json.dumps(line), flush=True)
 
 
+def relaunch_ranks(args):
+    """`python bench.py --gpus N` without torchrun: start the N ranks ourselves (one process per GPU,
+    rendezvous on 127.0.0.1), with the same arguments."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--points", type=int, default=N_FULL, help="points per GPU (config 3: 1e8)")
-    ap.add_argument("--e2e-points", type=int, default=N_FULL)
+    ap.add_argument("--e2e-points", type=int, default=N_FULL, help="points of the end-to-end leg, all ranks together")
     ap.add_argument("--ref-points", type=int, default=2_000_000, help="oracle sample per step")
     ap.add_argument("--parity", action="store_true", help="check every output of the batch against the oracle (~2 min)")
     ap.add_argument("--no-e2e", action="store_true")
@@ -397,6 +478,8 @@ def main():
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        relaunch_ranks(args)
     else:
         run_gpu(args)
 
