@@ -448,6 +448,44 @@ def run_gpu(args):
     print(json.dumps(line), flush=True)
 
 
+def run_leg(args):
+    """--leg NAME: one named workload, --warmup + --steps launches and nothing else -- the command the ncu
+    captures under profiles/ were taken with (one kernel family per capture)."""
+    import torch
+    from paper_2009_06635_b200 import binding as B, build
+    build.build()
+    grid = W.grid_nnpdf_shaped()
+    h = B.load_pdf_spec(grid)
+    p11 = list(W.PIDS_11)
+    dev = lambda *arrs: [torch.from_numpy(a).cuda() for a in arrs]
+    n4 = 10_000_000
+    if args.leg in ("config4", "config4_f1"):
+        x, q2 = dev(*W.queries_extrapolation_mix(grid, n4))
+        pids = p11 if args.leg == "config4" else [21]
+        o = torch.empty((len(pids), n4), dtype=torch.float64, device="cuda")
+        fn = lambda: B.pdf_xfxq2(h, pids, x, q2, o)
+    elif args.leg == "lumi":
+        x1, x2, q2 = dev(*W.queries_mc_events(grid, n4))
+        terms = [(q, -q, 1.0) for q in (1, 2, 3, 4, 5)] + [(-q, q, 1.0) for q in (1, 2, 3, 4, 5)] + [(21, 21, 0.25)]
+        lum = torch.empty(n4, dtype=torch.float64, device="cuda")
+        fn = lambda: B.pdf_lumi_events(h, terms, x1, x2, q2, lum)
+    elif args.leg == "alphas":
+        ha = B.load_alphas_spec(W.make_alphas_grid())
+        (q2,) = dev(W.queries_in_range(grid, args.points, 3)[1])
+        o = torch.empty_like(q2)
+        fn = lambda: B.alphas_q2(ha, q2, o)
+    elif args.leg == "members":
+        g0 = W.grid_member(0)
+        hs = B.pdf_set_load(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, W.member_values(args.members))
+        x, q2 = dev(*W.queries_fk_xgrid(g0))
+        o = torch.empty((args.members, 13, len(x)), dtype=torch.float64, device="cuda")
+        fn = lambda: B.pdf_xfxq2_members(hs, 0, args.members, list(W.PIDS_13), x, q2, o)
+    else:
+        raise SystemExit(f"unknown --leg {args.leg}")
+    t = timed_reps(torch, fn, reps=args.steps, warm=max(args.warmup, 1))
+    print(json.dumps({"leg": args.leg, **t}), flush=True)
+
+
 def relaunch_ranks(args):
     """`python bench.py --gpus N` without torchrun: start the N ranks ourselves (one process per GPU,
     rendezvous on 127.0.0.1), with the same arguments."""
@@ -475,9 +513,12 @@ def main():
     ap.add_argument("--no-members", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--members", type=int, default=400, help="N_rep of the multi-member leg (Table 2)")
+    ap.add_argument("--leg", default=None, help="profiling aid: run only config4 | config4_f1 | lumi | alphas | members")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.leg:
+        run_leg(args)
     elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         relaunch_ranks(args)
     else:

@@ -29,7 +29,8 @@ def needs_build() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
-        cmd = [NVCC] + FLAGS + ["-o", LIB] + sources()
+        extra = os.environ.get("PDFB_BUILD_FLAGS", "").split()  # e.g. -DPDFB_CHECKED: the bounds-checked build
+        cmd = [NVCC] + FLAGS + extra + ["-o", LIB] + sources()
         res = subprocess.run(cmd, capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)

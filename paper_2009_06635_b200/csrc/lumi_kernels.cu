@@ -102,6 +102,13 @@ k_lumi_band(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef 
         for (int e = tid; e < nqr; e += LUMI_NT) qr[e] = __ldg(src + npre + e);
         int4 *bz = reinterpret_cast<int4 *>(smem + L.l_band);
         for (int e = tid; e < NPAIR * L.pair_stride / 16; e += LUMI_NT) bz[e] = make_int4(0, 0, 0, 0);
+#ifdef PDFB_CHECKED
+        // poison what a band will overwrite (the rows of the pairs that exist): only a pair that does not exist
+        // and the alignment row keep their zeros
+        for (int p = 0; p < g.n_groups2; p++)
+            for (int e = tid; e < L.R * L.RB2 / 8; e += LUMI_NT)
+                reinterpret_cast<unsigned long long *>(smem + L.l_band + p * L.pair_stride)[e] = 0x7ff8dead00000000ULL;
+#endif
     }
     const long long n_tiles = (n + LUMI_NT - 1) / LUMI_NT;
     for (int band = 0; band < L.n_bands; band++) {
@@ -199,6 +206,7 @@ k_lumi_band(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef 
             if (m) {
                 if (mine) {
                     const int pos = cnt + __popc(m & ((1u << lane) - 1u));
+                    PDFB_ASSERT(pos < LUMI_LIST);
                     lx1[pos] = xa; lx2[pos] = xb; lq[pos] = qv; le[pos] = (uint32_t)e;
                 }
                 cnt += __popc(m);

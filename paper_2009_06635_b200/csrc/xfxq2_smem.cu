@@ -58,6 +58,14 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     }
     if (tid < NT_SMEM / 32 * 8) (&wcnt[0][0])[tid] = 0;
     if (tid < NT_SMEM / 32) s_req[tid] = 0;
+#ifdef PDFB_CHECKED
+    {   // poison the whole window: whatever is read later must have been staged
+        uint32_t size;
+        asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(size));
+        for (uint32_t e = tid; e < size / 8; e += NT_SMEM) reinterpret_cast<unsigned long long *>(smem)[e] = 0x7ff8dead00000000ULL;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+#endif
     __syncthreads();
     if (tid == 0) {
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(slice_bytes) : "memory");
@@ -180,6 +188,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                     unsigned char *cnt = &wcnt[threadIdx.x >> 5][cls];
                     const int cur = *cnt, kc = __popc(peers);
                     // (cur + kc <= TRIGGER - 1 + 32 + 31 < LCAP: the trigger below empties the list at the end of its tile)
+                    PDFB_ASSERT(cur + kc <= PDFB_SLOW_LCAP && p < n);
                     __stcg(wlist() + cls * PDFB_SLOW_LCAP + cur + __popc(peers & ((1u << lane) - 1u)), (uint32_t)p);
                     __syncwarp(slow_mask);
                     if ((peers & ((1u << lane) - 1u)) == 0) {  // the first lane of the class

@@ -17,8 +17,30 @@ struct PassList {
 #define PPT_SMEM 1    // points per thread and tile
 #endif
 
+// PDFB_CHECKED (build.py: PDFB_BUILD_FLAGS=-DPDFB_CHECKED): every shared-memory gather address is checked
+// against the dynamic shared-memory window of the CTA, and the kernels poison the window with NaN
+// before staging -- a read of anything that was not staged, even with weight 0, then shows up as a
+// NaN output.  (compute-sanitizer is closed on the pool this was developed on; profiles/r2_sanitizer.md.)
+#ifdef PDFB_CHECKED
+#include <cassert>
+__device__ __forceinline__ void pdfb_check_smem(uint32_t addr, uint32_t bytes)
+{
+    extern __shared__ __align__(128) unsigned char pdfb_dyn_smem[];  // every extern array is the dynamic window
+    uint32_t size;
+    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(size));
+    const uint32_t lo = (uint32_t)__cvta_generic_to_shared(pdfb_dyn_smem);
+    assert(addr % bytes == 0 && addr >= lo && addr + bytes <= lo + size);
+}
+#define PDFB_ASSERT(c) assert(c)
+#else
+#define PDFB_ASSERT(c)
+#endif
+
 __device__ __forceinline__ double2 lds128(uint32_t addr)
 {
+#ifdef PDFB_CHECKED
+    pdfb_check_smem(addr, 16);
+#endif
     double2 v;
     asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
     return v;
