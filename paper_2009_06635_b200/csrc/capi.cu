@@ -150,7 +150,8 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid * n_members, 128);
     size_t o_valg2 = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_members, 128);
     size_t o_aux = align_up(o_valg2 + (size_t)d.slice2_bytes * d.n_groups2 * n_members, 128);
-    size_t o_ws = align_up(o_aux + aux_bytes, 128);
+    size_t o_rr = align_up(o_aux + aux_bytes, 128);
+    size_t o_ws = align_up(o_rr + sizeof(int) * 2 * PDFB_RR_SLOTS, 128);
     size_t total = o_ws + PDFB_WS_BYTES;
     char *blob = nullptr;
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
@@ -246,6 +247,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.valg2 = (const double *)(blob + o_valg2);
     d.aux = (const unsigned char *)(blob + o_aux);
     d.slow_ws = (uint32_t *)(blob + o_ws);
+    d.row_range = (int *)(blob + o_rr);
     if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
     pdfb_lumi_plan(g);
     *out = g;

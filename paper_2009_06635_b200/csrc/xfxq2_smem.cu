@@ -32,28 +32,53 @@ template <int MODE, int W>  // compile-time (xfxq2_smem.cuh): a run-time flag co
 __global__ void __launch_bounds__(NT_SMEM, 1)
 k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
              const double *__restrict__ x, const double *__restrict__ q2, double *__restrict__ out,
-             long long out_stride, int member0, int n_req, int n_jobs)
+             long long out_stride, int member0, int n_req, int n_jobs, const int *__restrict__ row_range)
 {
     constexpr bool Q_IS_Q = MODE & 1;
-    constexpr int OUT = MODE >> 1;
+    constexpr int OUT = (MODE >> 1) & 3;
+    constexpr bool SETS = (MODE >> 3) & 1;  // persistent over jobs: more (member, pass) jobs than SMs
     extern __shared__ __align__(128) unsigned char smem[];
-    __shared__ __align__(8) unsigned long long mbar;
+    __shared__ __align__(8) unsigned long long mbar[2];  // the rows of buffer 0 / 1 have landed
     __shared__ unsigned char wcnt[NT_SMEM / 32][8];  // entries in each warp's class lists
     __shared__ __align__(16) unsigned char s_req[NT_SMEM / 32];  // "evaluate your full batches now", one flag per warp
     const int tid = threadIdx.x, lane = tid & 31;
-    // job = (member of the set, pass): blockIdx.x = seq * n_jobs + job; a job's CTAs share its tiles
-    const int job = blockIdx.x % n_jobs, seq = blockIdx.x / n_jobs, nseq = gridDim.x / n_jobs;
-    const int pass = job % pl.n, mem = job / pl.n;
-    // (the members of a set follow each other in `out`; fp32 output counts in floats)
-    out = (OUT == PDFB_OUT_FM32) ? reinterpret_cast<double *>(reinterpret_cast<float *>(out) + (long long)mem * n_req * out_stride)
-                                 : out + (long long)mem * n_req * out_stride;
-    const uint32_t tab = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)g.pre_bytes;
-    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&mbar);
+    // job = (member of the set, pass).  Few jobs: blockIdx.x = seq * n_jobs + job, a job's CTAs share its
+    // tiles.  SETS: CTA b takes jobs b, b + gridDim.x, ... over all tiles, the next job's rows in flight.
+    int job = SETS ? blockIdx.x : blockIdx.x % n_jobs;
+    const int seq = SETS ? 0 : blockIdx.x / n_jobs, nseq = SETS ? 1 : gridDim.x / n_jobs;
+    double *const out_base = out;
+    const uint32_t tab0 = (uint32_t)__cvta_generic_to_shared(smem) + (uint32_t)g.pre_bytes;
+    const uint32_t mb = (uint32_t)__cvta_generic_to_shared(&mbar[0]);
     const int slice_bytes = (W == 4) ? g.slice_bytes : g.slice2_bytes;
+    // small batches stage only the table rows their Q^2 values can touch (k_row_range below), at the
+    // rows' own places in the slice: nothing else of this kernel changes.  SETS: if twice that many rows
+    // fit, the odd jobs of a CTA use a second copy `shift` bytes further up (no point is outside the
+    // grid then, k_row_range: the out-of-grid classes, which locate the table themselves, never run).
+    const int RBs = (W == 4) ? g.nx4 * 32 : g.nx2 * 16;
+    const int r0 = row_range ? row_range[0] : 0, r1 = row_range ? row_range[1] : g.nq_tot;
+    const int lo = r0 * RBs, stage = (r1 - r0) * RBs;
+    int shift = 0;
+    if (SETS && row_range) {
+        const int rows = (r1 - r0 + 1) & ~1;  // even: the copy keeps the bank alignment of 2-column rows
+        if ((rows + r1) * RBs <= slice_bytes) shift = rows * RBs;
+    }
+    auto stage_job = [&](int j, int buf) {  // one thread: the rows of job j into buffer buf
+        const int ps = j % pl.n, mm = j / pl.n;
+        const uint32_t bar = mb + 8u * buf;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(stage) : "memory");
+        const unsigned char *src = reinterpret_cast<const unsigned char *>(W == 4 ? g.valg : g.valg2) +
+                                   ((size_t)(member0 + mm) * (W == 4 ? g.n_groups : g.n_groups2) + pl.group[ps]) * slice_bytes + lo;
+        for (int o = 0; o < stage; o += 32768) {
+            int bytes = min(32768, stage - o);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(tab0 + buf * shift + lo + o), "l"(src + o), "r"(bytes), "r"(bar) : "memory");
+        }
+    };
 
     // ---- stage this CTA's flavour-group slice with TMA bulk copies; small tables by plain loads
     if (tid == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb));
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(mb + 8u));
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (tid < NT_SMEM / 32 * 8) (&wcnt[0][0])[tid] = 0;
@@ -67,16 +92,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     }
 #endif
     __syncthreads();
-    if (tid == 0) {
-        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mb), "r"(slice_bytes) : "memory");
-        const unsigned char *src = reinterpret_cast<const unsigned char *>(W == 4 ? g.valg : g.valg2) +
-                                   ((size_t)(member0 + mem) * (W == 4 ? g.n_groups : g.n_groups2) + pl.group[pass]) * slice_bytes;
-        for (int o = 0; o < slice_bytes; o += 32768) {
-            int bytes = min(32768, slice_bytes - o);
-            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                         ::"r"(tab + o), "l"(src + o), "r"(bytes), "r"(mb) : "memory");
-        }
-    }
+    if (tid == 0) stage_job(job, 0);
     {   // pre and post blocks around the slice (both multiples of 128 bytes)
         const int4 *src = reinterpret_cast<const int4 *>(g.aux);
         int4 *pre = reinterpret_cast<int4 *>(smem), *post = reinterpret_cast<int4 *>(smem + g.pre_bytes + slice_bytes);
@@ -85,12 +101,23 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         for (int e = tid; e < npost; e += NT_SMEM) post[e] = __ldg(src + npre + e);
     }
     __syncthreads();
+    int jj = 0;
+    do {  // jobs of this CTA (one, unless SETS)
+    const int buf = shift ? (jj & 1) : 0;
+    // (the buffer of job jj - 1 is free: every warp passed the barrier at the end of that job)
+    if (SETS && shift && tid == 0 && job + (int)gridDim.x < n_jobs) stage_job(job + gridDim.x, buf ^ 1);
     {
         uint32_t done = 0;
+        const uint32_t parity = shift ? ((jj >> 1) & 1) : (jj & 1);
         while (!done)
-            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                         : "=r"(done) : "r"(mb) : "memory");
+            asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                         : "=r"(done) : "r"(mb + 8u * buf), "r"(parity) : "memory");
     }
+    const int pass = job % pl.n, mem = job / pl.n;
+    // (the members of a set follow each other in `out`; fp32 output counts in floats)
+    out = (OUT == PDFB_OUT_FM32) ? reinterpret_cast<double *>(reinterpret_cast<float *>(out_base) + (long long)mem * n_req * out_stride)
+                                 : out_base + (long long)mem * n_req * out_stride;
+    const uint32_t tab = tab0 + (uint32_t)(buf * shift);
     const SmemViews sv = make_views<W>(g, smem);
     const int lane8 = tid & 7;
     const uint32_t RB = sv.row_bytes, rb2 = 2u * RB, rb3 = 3u * RB;
@@ -207,12 +234,64 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     if (pending) { flush_lists(false); pending = false; }
     }
     flush_lists(true);
+    if (SETS) {
+        __syncthreads();  // every warp is done with this job's rows (measured: mbarrier hand-over between the warps
+                          // instead of this barrier changes nothing -- a job is bound by its five tile iterations)
+        if (!shift && tid == 0 && job + (int)gridDim.x < n_jobs) stage_job(job + gridDim.x, 0);  // one buffer: stage now
+    }
+    ++jj;
+    } while (SETS && (job += gridDim.x) < n_jobs);
+}
+
+// Rows of the concatenated Q^2 knot list that a batch can touch: the intervals of its smallest and
+// largest in-range Q^2, two rows below and three above (the 4-row stencils and their zero-weight
+// overreach); the whole table as soon as one point lies outside the grid (the out-of-grid classes read
+// fixed rows at either end and locate the table themselves).  (old text follows)
+// 
+// one Q^2 lies outside the grid (rules B and C read fixed rows at either end).  One CTA; for batches
+// small enough that staging the whole 200 KB slice per CTA costs as much as evaluating them
+// (PDF sets on an x-grid at one scale: 2415 points, 4 rows of 64).
+template <bool Q_IS_Q>
+__global__ void __launch_bounds__(1024) k_row_range(const GridDev g, long long n, const double *__restrict__ x,
+                                                    const double *__restrict__ q2, int *__restrict__ rr)
+{
+    __shared__ double smin[32], smax[32];
+    __shared__ int sout[32];
+    double lo = g.q2_max, hi = g.q2_min;
+    int outside = 0;
+    for (long long p = threadIdx.x; p < n; p += 1024) {
+        const double q = load_scale<Q_IS_Q>(q2 + p), xv = x[p];
+        if (!(xv > 0.0) || !(xv <= g.x_max) || !(q > 0.0) || isinf(q)) continue;  // no value: touches no row
+        if (q >= g.q2_min && q <= g.q2_max) { lo = fmin(lo, q); hi = fmax(hi, q); }
+        if (q < g.q2_min || q > g.q2_max || xv < g.x_min) outside = 1;
+    }
+    for (int o = 16; o; o >>= 1) {
+        lo = fmin(lo, __shfl_xor_sync(0xffffffffu, lo, o)); hi = fmax(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        outside |= __shfl_xor_sync(0xffffffffu, outside, o);
+    }
+    if ((threadIdx.x & 31) == 0) { smin[threadIdx.x >> 5] = lo; smax[threadIdx.x >> 5] = hi; sout[threadIdx.x >> 5] = outside; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < 32; w++) { lo = fmin(lo, smin[w]); hi = fmax(hi, smax[w]); outside |= sout[w]; }
+        int r0 = 0, r1 = g.nq_tot;
+        if (!outside && lo <= hi) {
+            int a = 0, b = 0;  // intervals of lo and hi: the last knot <= the value (a threshold: its upper copy)
+            for (int m = 1; m < g.nq_tot; m++) { if (g.q2k[m] <= lo) a = m; if (g.q2k[m] <= hi) b = m; }
+            b = min(b, g.nq_tot - 2);
+            // rows a-1 .. b+2 hold the stencils; knot -1 of a row is the tail of the row below and knot nx of a
+            // row the head of the row above (weight exactly 0, but they must be staged, finite data): one more each
+            r0 = max(a - 2, 0); r1 = min(b + 4, g.nq_tot);
+        } else if (!outside) { r1 = 1; }  // no point with a value: nothing to stage but a row of finite data
+        rr[0] = r0; rr[1] = r1;
+    }
 }
 
 // Dynamic shared memory of a launch.  Never less than PDFB_SMEM_FLOOR (more than half of the SM's
 // 228 KB): two CTAs of this kernel can then not be resident on one SM, whatever the grid size, the
 // register count or the stream -- the invariant the per-SM scratch slot of the class lists rests on.
 static const int PDFB_SMEM_FLOOR = 116 * 1024;
+static const long long PDFB_RR_MAX_POINTS = 65536;  // batches up to this size look for their row range first ...
+static const int PDFB_RR_MIN_SLICE = 64 * 1024;      // ... if a slice is at least this big
 static int smem_image(const GridDev &d, int W) { return d.pre_bytes + (W == 4 ? d.slice_bytes : d.slice2_bytes) + d.post_bytes; }
 static int smem_needed(const GridDev &d, int W) { const int b = smem_image(d, W); return b > PDFB_SMEM_FLOOR ? b : PDFB_SMEM_FLOOR; }
 static const int STATIC_SMEM = 256;  // >= the kernel's static shared memory (mbarrier, list counters)
@@ -239,6 +318,7 @@ int pdfb_smem_eligible(const pdfb_grid *g)
 #define PDFB_ATTR(M, WW) if (e == cudaSuccess) e = cudaFuncSetAttribute(k_xfxq2_smem<M, WW>, cudaFuncAttributeMaxDynamicSharedMemorySize, lim)
         PDFB_ATTR(0, 4); PDFB_ATTR(1, 4); PDFB_ATTR(2, 4); PDFB_ATTR(4, 4);
         PDFB_ATTR(0, 2); PDFB_ATTR(1, 2); PDFB_ATTR(2, 2); PDFB_ATTR(4, 2);
+        PDFB_ATTR(8, 4); PDFB_ATTR(9, 4); PDFB_ATTR(8, 2); PDFB_ATTR(9, 2);
 #undef PDFB_ATTR
         if (e != cudaSuccess) {
             cudaGetLastError();
@@ -300,6 +380,15 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     const long long n_jobs = (long long)pl.n * n_mem;
     if (n_jobs > 0x3fffffff) return PDFB_ELIMIT;
     const int smem = smem_needed(g->d, W);
+    // small batch on a big slice: find the rows it needs first (one more launch of a single CTA)
+    const int *rr = nullptr;
+    if (n <= PDFB_RR_MAX_POINTS && (W == 4 ? g->d.slice_bytes : g->d.slice2_bytes) >= PDFB_RR_MIN_SLICE) {
+        int *slot = g->d.row_range + 2 * (const_cast<pdfb_grid *>(g)->rr_next.fetch_add(1, std::memory_order_relaxed) % PDFB_RR_SLOTS);
+        if (mode & 1) k_row_range<true><<<1, 1024, 0, st>>>(g->d, n, x, q2, slot);
+        else k_row_range<false><<<1, 1024, 0, st>>>(g->d, n, x, q2, slot);
+        pdfb_count_launch(1);
+        rr = slot;
+    }
     // the class lists hold point indices as 32-bit offsets: batches beyond 2^31 points go out in slices
     const long long SLICE = 1LL << 31;
     for (long long off = 0; off < n; off += SLICE) {
@@ -308,12 +397,17 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
         if (per_job < 1) per_job = 1;
         const long long tiles = (m + NT_SMEM * PPT_SMEM - 1) / (NT_SMEM * PPT_SMEM);
         if (per_job > tiles) per_job = (int)tiles;
-        const unsigned grid = (unsigned)(per_job * n_jobs);
-#define PDFB_LAUNCH(M, WW) k_xfxq2_smem<M, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, m, x + off, q2 + off, out_off, out_stride, member0, n_req, (int)n_jobs)
+        // more jobs than SMs (PDF sets): one persistent CTA per SM walks the jobs, the next job's rows in flight
+        const bool sets = n_jobs > sms && mode <= 1;
+        const unsigned grid = sets ? (unsigned)sms : (unsigned)(per_job * n_jobs);
+#define PDFB_LAUNCH(M, WW) k_xfxq2_smem<M, WW><<<grid, NT_SMEM, smem, st>>>(g->d, pl, m, x + off, q2 + off, out_off, out_stride, member0, n_req, (int)n_jobs, rr)
         // element offset of this slice in `out` (doubles, or floats for the fp32 variant)
         const long long eo = (mode >> 1) == PDFB_OUT_PM64 ? off * n_req : off;
         double *out_off = (mode >> 1) == PDFB_OUT_FM32 ? reinterpret_cast<double *>(reinterpret_cast<float *>(out) + eo) : out + eo;
-        if (W == 4) { if (mode == 0) PDFB_LAUNCH(0, 4); else if (mode == 1) PDFB_LAUNCH(1, 4); else if (mode == 2) PDFB_LAUNCH(2, 4); else PDFB_LAUNCH(4, 4); }
+        if (sets) {
+            if (W == 4) { if (mode == 0) PDFB_LAUNCH(8, 4); else PDFB_LAUNCH(9, 4); }
+            else        { if (mode == 0) PDFB_LAUNCH(8, 2); else PDFB_LAUNCH(9, 2); }
+        } else if (W == 4) { if (mode == 0) PDFB_LAUNCH(0, 4); else if (mode == 1) PDFB_LAUNCH(1, 4); else if (mode == 2) PDFB_LAUNCH(2, 4); else PDFB_LAUNCH(4, 4); }
         else        { if (mode == 0) PDFB_LAUNCH(0, 2); else if (mode == 1) PDFB_LAUNCH(1, 2); else if (mode == 2) PDFB_LAUNCH(2, 2); else PDFB_LAUNCH(4, 2); }
 #undef PDFB_LAUNCH
         pdfb_count_launch(1);
