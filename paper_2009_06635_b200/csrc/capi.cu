@@ -116,7 +116,8 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.x_min = x_knots[0]; d.x_max = x_knots[nx - 1];
     d.q2_min = h_q2[0]; d.q2_max = h_q2[nq_tot - 1];
 
-    // one device blob: [xk | q2k | z (ln knots) | xrec | qrec | val | raw values | counter]
+    // one device blob: [xk | q2k | z (ln knots) | xrec | qrec | val | counter | valg | valg2 | aux | row ranges | lists];
+    // the uploaded file-order values live in a staging allocation of their own, freed after K1
     size_t o_xk = 0;
     size_t o_q2k = align_up(o_xk + sizeof(double) * nx, 128);
     size_t o_z = align_up(o_q2k + sizeof(double) * (nq_tot + 1), 128);
@@ -124,8 +125,6 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     size_t o_qrec = align_up(o_xrec + sizeof(IntervalRec) * nx, 128);
     size_t o_val = align_up(o_qrec + sizeof(IntervalRec) * nq_tot, 128);
     d.val_mstride = knots * d.kpad;  // one member's table, in doubles
-    size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad * n_members, 128);
-    size_t o_raw = align_up(o_cnt + 128, 128);
     // shared-memory path: flavour-group slices and the aux block
     d.nx4 = (nx + 3) & ~3;
     d.n_groups = (n_pid + 3) / 4;
@@ -147,14 +146,24 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.post_bytes = (int)align_up((size_t)std::max(128 * nq_tot, d.nx4 * 32 + 128), 128);
     if (128 * nx < d.nx4 * 32 + 32) d.smem_ok = 0;  // (never: 128 nx >= 32 nx4 + 32 for nx >= 2)
     const int aux_bytes = d.pre_bytes + d.post_bytes;
-    size_t o_valg = align_up(o_raw + sizeof(double) * knots * n_pid * n_members, 128);
-    size_t o_valg2 = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_members, 128);
-    size_t o_aux = align_up(o_valg2 + (size_t)d.slice2_bytes * d.n_groups2 * n_members, 128);
+    // which layouts this handle will ever read (a set of 400 members is ~1 GB if all are kept):
+    // the shared-memory path takes the 4-column slices (bit 0) and / or the 2-column slices (bit 1);
+    // the [iq][ix][kpad] table serves the read-only-cache kernel -- every member if that kernel is the
+    // only path, else member 0 alone (the general kernel of pdf_lumi_events)
+    if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
+    const int n_val = d.smem_ok ? 1 : n_members;
+    const int n_g4 = (d.smem_ok & 1) ? n_members : 0, n_g2 = (d.smem_ok & 2) ? n_members : 0;
+    size_t o_cnt = align_up(o_val + sizeof(double) * knots * d.kpad * n_val, 128);
+    size_t o_valg = align_up(o_cnt + 128, 128);
+    size_t o_valg2 = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_g4, 128);
+    size_t o_aux = align_up(o_valg2 + (size_t)d.slice2_bytes * d.n_groups2 * n_g2, 128);
     size_t o_rr = align_up(o_aux + aux_bytes, 128);
     size_t o_ws = align_up(o_rr + sizeof(int) * 2 * PDFB_RR_SLOTS, 128);
     size_t total = o_ws + PDFB_WS_BYTES;
-    char *blob = nullptr;
+    char *blob = nullptr, *raw = nullptr;
+    const long long member_values = knots * n_pid;  // doubles of one member in file order
     if (cudaMalloc(&blob, total) != cudaSuccess) { delete g; return PDFB_ECUDA; }
+    if (cudaMalloc(&raw, sizeof(double) * member_values * n_members) != cudaSuccess) { cudaFree(blob); delete g; return PDFB_ECUDA; }
     g->blob = blob; g->blob_bytes = total;
 
     int rc = PDFB_OK;
@@ -167,7 +176,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     do {
         if (cudaMemcpy(blob + o_xk, x_knots, sizeof(double) * nx, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(blob + o_q2k, h_q2.data(), sizeof(double) * (nq_tot + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
-            cudaMemcpy(blob + o_raw, values, sizeof(double) * knots * n_pid * n_members, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(raw, values, sizeof(double) * member_values * n_members, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemset(blob + o_cnt, 0, 128) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         cudaEventRecord(e0, 0);
         // K1: ln of the knots (and of rule C's probe scale), read back for the host-side tables
@@ -198,24 +207,19 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
         rc = pdfb_setup_records((const double *)(blob + o_z) + nx, (IntervalRec *)(blob + o_qrec),
                                 (IntervalRec32 *)(blob + o_aux + d.pre_bytes + d.a_qrec), n_sub, d.q_off, 0);
         if (rc) break;
-        // K1: value table re-layout, member by member, sub-grid by sub-grid
+        // K1: value table re-layout, sub-grid by sub-grid, all members of a layout in one launch
         long long src = 0;
-        for (int m = 0; m < n_members && !rc; m++) {
-            double *valg_m = (double *)(blob + o_valg) + (long long)m * d.n_groups * (d.slice_bytes / 8);
-            for (int s = 0; s < n_sub && !rc; s++) {
-                int nq = q_offsets[s + 1] - q_offsets[s];
-                rc = pdfb_setup_values((const double *)(blob + o_raw) + src,
-                                       (double *)(blob + o_val) + m * d.val_mstride + (long long)d.v_off[s] * d.kpad,
-                                       nx, nq, n_pid, d.kpad, 0);
-                if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src, valg_m,
-                                                      q_offsets[s] * d.nx4, nx, d.nx4, nq, n_pid, d.n_groups,
-                                                      (long long)d.slice_bytes / 8, 0);
-                if (!rc) rc = pdfb_setup_group_slices((const double *)(blob + o_raw) + src,
-                                                      (double *)(blob + o_valg2) + (long long)m * d.n_groups2 * (d.slice2_bytes / 8),
-                                                      q_offsets[s] * d.nx2, nx, d.nx2, nq, n_pid, d.n_groups2,
-                                                      (long long)d.slice2_bytes / 8, 0, 2);
-                src += (long long)nx * nq * n_pid;
-            }
+        for (int s = 0; s < n_sub && !rc; s++) {
+            int nq = q_offsets[s + 1] - q_offsets[s];
+            rc = pdfb_setup_values((const double *)raw + src, (double *)(blob + o_val) + (long long)d.v_off[s] * d.kpad,
+                                   nx, nq, n_pid, d.kpad, 0, n_val, member_values, d.val_mstride);
+            if (!rc && n_g4) rc = pdfb_setup_group_slices((const double *)raw + src, (double *)(blob + o_valg),
+                                                          q_offsets[s] * d.nx4, nx, d.nx4, nq, n_pid, d.n_groups,
+                                                          (long long)d.slice_bytes / 8, 0, 4, n_g4, member_values);
+            if (!rc && n_g2) rc = pdfb_setup_group_slices((const double *)raw + src, (double *)(blob + o_valg2),
+                                                          q_offsets[s] * d.nx2, nx, d.nx2, nq, n_pid, d.n_groups2,
+                                                          (long long)d.slice2_bytes / 8, 0, 2, n_g2, member_values);
+            src += (long long)nx * nq * n_pid;
         }
         if (rc) break;
         cudaEventRecord(e1, 0);
@@ -235,6 +239,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
         weights4(rC, (h_z[nx + nq_tot] - rC.z0) * rC.inv_dz, d.wvC);
     } while (0);
     cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(raw);  // (the device is idle: synchronised above, or setup failed)
     if (rc) { cudaFree(blob); delete g; return rc; }
 
     d.xk = (const double *)(blob + o_xk);
@@ -248,7 +253,6 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.aux = (const unsigned char *)(blob + o_aux);
     d.slow_ws = (uint32_t *)(blob + o_ws);
     d.row_range = (int *)(blob + o_rr);
-    if (d.smem_ok) d.smem_ok = pdfb_smem_eligible(g);
     pdfb_lumi_plan(g);
     *out = g;
     return PDFB_OK;

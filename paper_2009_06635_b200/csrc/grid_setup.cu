@@ -71,8 +71,11 @@ __global__ void k1_interval_records(const double *__restrict__ z, IntervalRec *_
 // (the shared-memory path stages one slice per CTA; W = 4 or 2 columns per group, nxp = padded
 // knots per row); padding columns / knots = 0
 __global__ void k1_group_slices(const double *__restrict__ src, double *__restrict__ valg, int s_knot_off,
-                                int nx, int nxp, int nq, int n_pid, int n_groups, long long group_stride, int W)
+                                int nx, int nxp, int nq, int n_pid, int n_groups, long long group_stride, int W,
+                                long long src_mstride)
 {
+    src += blockIdx.y * src_mstride;                      // blockIdx.y = member of the set
+    valg += blockIdx.y * (long long)n_groups * group_stride;
     long long tot = (long long)n_groups * nq * nxp * W;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
          e += (long long)gridDim.x * blockDim.x) {
@@ -89,8 +92,10 @@ __global__ void k1_group_slices(const double *__restrict__ src, double *__restri
 
 // values of one sub-grid: file order [ix][iq][ipid] -> [iq][ix][kpad], padding columns = 0
 __global__ void k1_relayout_values(const double *__restrict__ src, double *__restrict__ dst, int nx,
-                                   int nq, int n_pid, int kpad)
+                                   int nq, int n_pid, int kpad, long long src_mstride, long long dst_mstride)
 {
+    src += blockIdx.y * src_mstride;                      // blockIdx.y = member of the set
+    dst += blockIdx.y * dst_mstride;
     long long tot = (long long)nx * nq * kpad;
     for (long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x; e < tot;
          e += (long long)gridDim.x * blockDim.x) {
@@ -115,24 +120,25 @@ int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_r
 }
 
 int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
-                      cudaStream_t st)
+                      cudaStream_t st, int n_members, long long src_mstride, long long dst_mstride)
 {
     long long tot = (long long)nx * nq * kpad;
     int blocks = (int)((tot + 255) / 256);
     if (blocks > 1184) blocks = 1184;
-    k1_relayout_values<<<blocks, 256, 0, st>>>(d_src, d_dst, nx, nq, n_pid, kpad);
+    k1_relayout_values<<<dim3(blocks, n_members), 256, 0, st>>>(d_src, d_dst, nx, nq, n_pid, kpad, src_mstride, dst_mstride);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;
 }
 
 int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
-                            int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W)
+                            int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W, int n_members,
+                            long long src_mstride)
 {
     long long tot = (long long)n_groups * nq * nx4 * W;
     int blocks = (int)((tot + 255) / 256);
     if (blocks > 1184) blocks = 1184;
-    k1_group_slices<<<blocks, 256, 0, st>>>(d_src, d_valg, s_knot_off, nx, nx4, nq, n_pid, n_groups, group_stride, W);
+    k1_group_slices<<<dim3(blocks, n_members), 256, 0, st>>>(d_src, d_valg, s_knot_off, nx, nx4, nq, n_pid, n_groups, group_stride, W, src_mstride);
     pdfb_count_launch(1);
     PDFB_CUDA(cudaGetLastError());
     return PDFB_OK;

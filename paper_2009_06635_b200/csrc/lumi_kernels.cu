@@ -270,7 +270,7 @@ int pdfb_lumi_plan(pdfb_grid *g)
     memset(&L, 0, sizeof(L));
     g->lumi_npair = 0;
     const GridDev &d = g->d;
-    if (!d.smem_ok || d.n_members != 1) return PDFB_OK;  // general kernel only
+    if (!(d.smem_ok & 2)) return PDFB_OK;  // no 2-column slices: general kernel only (a set: its member 0)
     int npair = 0;
     for (int c : {2, 4, 6, 7}) if (d.n_groups2 <= c) { npair = c; break; }
     if (!npair) return PDFB_OK;

@@ -279,7 +279,8 @@ int pdfb_launch_alphas(const pdfb_alphas *a, long long n, const double *q2, doub
 int pdfb_setup_records(const double *d_z, IntervalRec *d_rec, IntervalRec32 *d_rec32, int n_arrays,
                        const int *h_off, cudaStream_t st);
 int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off, int nx, int nx4, int nq,
-                            int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W = 4);
+                            int n_pid, int n_groups, long long group_stride, cudaStream_t st, int W, int n_members,
+                            long long src_mstride);
 int pdfb_smem_eligible(const pdfb_grid *g);
 int pdfb_lumi_plan(pdfb_grid *g);
 int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long long n, const double *x,
@@ -290,7 +291,7 @@ int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, const do
                            const double2 *d_lntab, int n_sub, const int *h_off, cudaStream_t st);
 #define PDFB_ALPHAS_LINE 384   // bytes per interval in the fast-path image
 int pdfb_setup_values(const double *d_src, double *d_dst, int nx, int nq, int n_pid, int kpad,
-                      cudaStream_t st);
+                      cudaStream_t st, int n_members, long long src_mstride, long long dst_mstride);
 
 #define PDFB_CUDA(call)                          \
     do {                                         \
