@@ -28,9 +28,9 @@ METRIC = "pdf_evaluations_per_sec"
 UNIT = "evaluations/s"
 N_FULL = 100_000_000
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_xfxq2_smem launch at 1e8 points x 11
-# flavours, from the `ncu --set full` capture summarised in profiles/r1_xfxq2_smem_full.md
-NCU_TRAFFIC_BYTES_PER_POINT = (1.605477e9 + 8.741274e9) / 1e8
-NCU_TRAFFIC_SOURCE = "profiles/r1_xfxq2_smem_full.md (ncu, 1e8 points; scaled by points)"
+# flavours, from the `ncu --set full` capture summarised in profiles/r2_kernels.md
+NCU_TRAFFIC_BYTES_PER_POINT = (1.612596e9 + 8.742418e9) / 1e8
+NCU_TRAFFIC_SOURCE = "profiles/r2_kernels.md (ncu --set full, 1e8 points; scaled by points)"
 
 
 def measured_peaks():
