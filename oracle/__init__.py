@@ -37,6 +37,9 @@ def _load():
         lib.oracle_pdf_grid_create.restype = ctypes.c_void_p
         lib.oracle_pdf_grid_create.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _ip, _dp,
                                                ctypes.c_int, _ip, _dp]
+        lib.oracle_pdf_grid_create_xs.restype = ctypes.c_void_p
+        lib.oracle_pdf_grid_create_xs.argtypes = [ctypes.c_int, ctypes.c_int, _ip, _dp, _ip, _dp,
+                                                  ctypes.c_int, _ip, _dp]
         lib.oracle_pdf_grid_free.argtypes = [ctypes.c_void_p]
         lib.oracle_pdf_grid_invalid.restype = ctypes.c_long
         lib.oracle_pdf_grid_invalid.argtypes = [ctypes.c_void_p]
@@ -79,18 +82,28 @@ def ln(a: float) -> float:
 class OraclePdfGrid:
     """Oracle-side grid (arguments as in the C-ABI's pdf_grid_load)."""
 
-    def __init__(self, x_knots, q_offsets, q_knots, pids, values):
+    def __init__(self, x_knots, q_offsets, q_knots, pids, values, x_offsets=None):
+        """x_offsets (n_sub + 1 entries into x_knots): every sub-grid has its own x-knot array and the
+        values are [s][ix_s][iq_s][ipid]; None: one x-knot array shared by all sub-grids."""
         lib = _load()
         x_knots, q_knots, values = _f64(x_knots), _f64(q_knots), _f64(values)
         q_offsets, pids = _i32(q_offsets), _i32(pids)
-        self._h = lib.oracle_pdf_grid_create(
-            len(q_offsets) - 1, len(x_knots), x_knots.ctypes.data_as(_dp),
-            q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
-            pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp))
+        if x_offsets is None:
+            self._h = lib.oracle_pdf_grid_create(
+                len(q_offsets) - 1, len(x_knots), x_knots.ctypes.data_as(_dp),
+                q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
+                pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp))
+        else:
+            x_offsets = _i32(x_offsets)
+            self._h = lib.oracle_pdf_grid_create_xs(
+                len(q_offsets) - 1, 0, x_offsets.ctypes.data_as(_ip), x_knots.ctypes.data_as(_dp),
+                q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
+                pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp))
 
     @classmethod
     def from_spec(cls, spec):
-        return cls(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, spec.values)
+        return cls(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, spec.values,
+                   x_offsets=getattr(spec, "x_offsets", None))
 
     def xfxq2(self, pids, x, q2, with_scale: bool = False):
         """-> out[n_req, n] (flavour-major); with_scale also returns the conditioning scale."""

@@ -45,8 +45,10 @@ static double ln_cr(double a) { return (double)logq((__float128)a); }
 /* ------------------------------------------------------------------ grid storage */
 typedef struct {
     int n_sub, nx, n_pid, nq_tot;
-    double *x;      /* [nx] x knots */
-    double *U;      /* [nx] ln x knots */
+    int *x_off;     /* [n_sub+1] subgrid s owns x knots x_off[s] .. x_off[s+1]-1 (LHAPDF lets every subgrid
+                       carry its own x-knot array; with one shared array all subgrids point at it) */
+    double *x;      /* x knots, per subgrid */
+    double *U;      /* ln x knots */
     int *q_off;     /* [n_sub+1] */
     double *q2;     /* [nq_tot] Q^2 knots, q2 = Q*Q */
     double *V;      /* [nq_tot] ln Q^2 knots */
@@ -57,6 +59,9 @@ typedef struct {
 } ogrid;
 
 static int nq_of(const ogrid *g, int s) { return g->q_off[s + 1] - g->q_off[s]; }
+static int nx_of(const ogrid *g, int s) { return g->x_off[s + 1] - g->x_off[s]; }
+static const double *x_of(const ogrid *g, int s) { return g->x + g->x_off[s]; }
+static const double *U_of(const ogrid *g, int s) { return g->U + g->x_off[s]; }
 
 /* f[i][m][k] of subgrid s */
 static double fval(const ogrid *g, int s, int i, int m, int k)
@@ -64,15 +69,25 @@ static double fval(const ogrid *g, int s, int i, int m, int k)
     return g->val[g->v_off[s] + ((long)i * nq_of(g, s) + m) * g->n_pid + k];
 }
 
-void *oracle_pdf_grid_create(int n_sub, int nx, const double *x_knots, const int *q_offsets,
-                             const double *q_knots, int n_pid, const int *pids,
-                             const double *values)
+/* x_offsets: [n_sub+1] into x_knots (per-subgrid x-knot arrays, values [s][ix_s][iq_s][ipid]), or NULL:
+ * one array of nx knots shared by all subgrids.  All subgrids must span the same [x_0, x_max]. */
+void *oracle_pdf_grid_create_xs(int n_sub, int nx, const int *x_offsets, const double *x_knots, const int *q_offsets,
+                                const double *q_knots, int n_pid, const int *pids,
+                                const double *values)
 {
     ogrid *g = (ogrid *)calloc(1, sizeof(ogrid));
-    g->n_sub = n_sub; g->nx = nx; g->n_pid = n_pid; g->nq_tot = q_offsets[n_sub];
-    g->x = (double *)malloc(sizeof(double) * nx);
-    g->U = (double *)malloc(sizeof(double) * nx);
-    for (int i = 0; i < nx; i++) { g->x[i] = x_knots[i]; g->U[i] = ln_cr(x_knots[i]); }
+    g->n_sub = n_sub; g->n_pid = n_pid; g->nq_tot = q_offsets[n_sub];
+    g->x_off = (int *)malloc(sizeof(int) * (n_sub + 1));
+    int nxt = x_offsets ? x_offsets[n_sub] : nx;
+    g->nx = nxt;
+    g->x = (double *)malloc(sizeof(double) * nxt * (x_offsets ? 1 : n_sub));
+    g->U = (double *)malloc(sizeof(double) * nxt * (x_offsets ? 1 : n_sub));
+    for (int s = 0; s <= n_sub; s++) g->x_off[s] = x_offsets ? x_offsets[s] : s * nx;
+    for (int s = 0; s < n_sub; s++)
+        for (int i = 0; i < nx_of(g, s); i++) {
+            double xv = x_offsets ? x_knots[x_offsets[s] + i] : x_knots[i];
+            g->x[g->x_off[s] + i] = xv; g->U[g->x_off[s] + i] = ln_cr(xv);
+        }
     g->q_off = (int *)malloc(sizeof(int) * (n_sub + 1));
     memcpy(g->q_off, q_offsets, sizeof(int) * (n_sub + 1));
     g->q2 = (double *)malloc(sizeof(double) * g->nq_tot);
@@ -85,17 +100,24 @@ void *oracle_pdf_grid_create(int n_sub, int nx, const double *x_knots, const int
     memcpy(g->pids, pids, sizeof(int) * n_pid);
     g->v_off = (long *)malloc(sizeof(long) * n_sub);
     long tot = 0;
-    for (int s = 0; s < n_sub; s++) { g->v_off[s] = tot; tot += (long)nx * nq_of(g, s) * n_pid; }
+    for (int s = 0; s < n_sub; s++) { g->v_off[s] = tot; tot += (long)nx_of(g, s) * nq_of(g, s) * n_pid; }
     g->val = (double *)malloc(sizeof(double) * tot);
     memcpy(g->val, values, sizeof(double) * tot);
     return g;
+}
+
+void *oracle_pdf_grid_create(int n_sub, int nx, const double *x_knots, const int *q_offsets,
+                             const double *q_knots, int n_pid, const int *pids,
+                             const double *values)
+{
+    return oracle_pdf_grid_create_xs(n_sub, nx, NULL, x_knots, q_offsets, q_knots, n_pid, pids, values);
 }
 
 void oracle_pdf_grid_free(void *h)
 {
     ogrid *g = (ogrid *)h;
     if (!g) return;
-    free(g->x); free(g->U); free(g->q_off); free(g->q2); free(g->V);
+    free(g->x); free(g->U); free(g->x_off); free(g->q_off); free(g->q2); free(g->V);
     free(g->pids); free(g->v_off); free(g->val); free(g);
 }
 
@@ -134,9 +156,10 @@ static cell locate(const ogrid *g, double x, double q2)
         if (g->q2[g->q_off[s]] <= q2) c.s = s;
     /* 2. cell: largest knot index <= the coordinate, clamped to the last interval;
      *    comparisons on raw x and Q^2, never on logs */
+    const double *xs = x_of(g, c.s), *Us = U_of(g, c.s);  /* the x knots of the point's own subgrid */
     c.i = 0;
-    for (int m = 1; m <= g->nx - 2; m++)
-        if (g->x[m] <= x) c.i = m;
+    for (int m = 1; m <= nx_of(g, c.s) - 2; m++)
+        if (xs[m] <= x) c.i = m;
     const double *q2s = g->q2 + g->q_off[c.s];
     int nq = nq_of(g, c.s);
     c.j = 0;
@@ -145,8 +168,8 @@ static cell locate(const ogrid *g, double x, double q2)
     /* 3. u = ln x, v = ln Q^2 */
     const double *Vs = g->V + g->q_off[c.s];
     double u = ln_cr(x), v = ln_cr(q2);
-    c.dU = g->U[c.i + 1] - g->U[c.i];
-    c.t = (u - g->U[c.i]) / c.dU;
+    c.dU = Us[c.i + 1] - Us[c.i];
+    c.t = (u - Us[c.i]) / c.dU;
     c.dV = Vs[c.j + 1] - Vs[c.j];
     c.tau = (v - Vs[c.j]) / c.dV;
     return c;
@@ -155,8 +178,8 @@ static cell locate(const ogrid *g, double x, double q2)
 /* O2 along x at fixed Q row m of subgrid s, for PID column k */
 static double du_at(const ogrid *g, int s, int i, int m, int k)
 {
-    const double *U = g->U;
-    int nx = g->nx;
+    const double *U = U_of(g, s);
+    int nx = nx_of(g, s);
     if (i == 0) return fd_slope(fval(g, s, 0, m, k), fval(g, s, 1, m, k), U[0], U[1]);
     if (i == nx - 1) return fd_slope(fval(g, s, nx - 2, m, k), fval(g, s, nx - 1, m, k), U[nx - 2], U[nx - 1]);
     return 0.5 * (fd_slope(fval(g, s, i, m, k), fval(g, s, i + 1, m, k), U[i], U[i + 1]) +
@@ -212,10 +235,20 @@ static double continuation(double z, double zL, double zH, double yL, double yH)
 }
 
 /* O5-A: x < x_0, Q^2 in range */
+/* subgrid of an in-range scale (O3 step 1) */
+static int subgrid_of(const ogrid *g, double q2)
+{
+    int s0 = 0;
+    for (int s = 1; s < g->n_sub; s++)
+        if (g->q2[g->q_off[s]] <= q2) s0 = s;
+    return s0;
+}
+
 static double rule_a(const ogrid *g, int k, double x, double q2)
 {
-    double yL = o3(g, k, g->x[0], q2), yH = o3(g, k, g->x[1], q2);
-    return continuation(ln_cr(x), g->U[0], g->U[1], yL, yH);
+    int s = subgrid_of(g, q2);  /* the first two x knots of the subgrid the scale falls in */
+    double yL = o3(g, k, x_of(g, s)[0], q2), yH = o3(g, k, x_of(g, s)[1], q2);
+    return continuation(ln_cr(x), U_of(g, s)[0], U_of(g, s)[1], yL, yH);
 }
 
 /* G(x, q): O3 if x >= x_0, rule A otherwise (q in range) */
@@ -246,7 +279,7 @@ static double rule_c(const ogrid *g, int k, double x, double q2)
 /* xf of PID column k at any (x, Q^2); NaN (and *bad = 1) where no value is defined */
 static double xf_any(const ogrid *g, int k, double x, double q2, int *bad)
 {
-    double xmax = g->x[g->nx - 1], qmin = g->q2[0], qmax = g->q2[g->nq_tot - 1];
+    double xmax = x_of(g, 0)[nx_of(g, 0) - 1], qmin = g->q2[0], qmax = g->q2[g->nq_tot - 1];
     if (!(x > 0.0) || !(q2 > 0.0) || !(x <= xmax) || isinf(q2)) { *bad = 1; return NAN; }
     if (q2 > qmax) return rule_b(g, k, x, q2);
     if (q2 < qmin) return rule_c(g, k, x, q2);
@@ -278,8 +311,8 @@ static double habs(double t, double yL, double dL, double yH, double dH)
 static double aslope(double yL, double yH, double zL, double zH) { return (fabs(yH) + fabs(yL)) / (zH - zL); }
 static double du_abs(const ogrid *g, int s, int i, int m, int k)
 {
-    const double *U = g->U;
-    int nx = g->nx;
+    const double *U = U_of(g, s);
+    int nx = nx_of(g, s);
     if (i == 0) return aslope(fval(g, s, 0, m, k), fval(g, s, 1, m, k), U[0], U[1]);
     if (i == nx - 1) return aslope(fval(g, s, nx - 2, m, k), fval(g, s, nx - 1, m, k), U[nx - 2], U[nx - 1]);
     return 0.5 * (aslope(fval(g, s, i, m, k), fval(g, s, i + 1, m, k), U[i], U[i + 1]) +
@@ -316,12 +349,14 @@ static double cont_scale(double z, double zL, double zH, double yL, double yH, d
 static double G_scale(const ogrid *g, int k, double x, double q2)
 {
     if (x >= g->x[0]) return o3_scale(g, k, x, q2);
-    return cont_scale(ln_cr(x), g->U[0], g->U[1], o3(g, k, g->x[0], q2), o3(g, k, g->x[1], q2),
-                      o3_scale(g, k, g->x[0], q2), o3_scale(g, k, g->x[1], q2));
+    int s = subgrid_of(g, q2);
+    const double *xs = x_of(g, s), *Us = U_of(g, s);
+    return cont_scale(ln_cr(x), Us[0], Us[1], o3(g, k, xs[0], q2), o3(g, k, xs[1], q2),
+                      o3_scale(g, k, xs[0], q2), o3_scale(g, k, xs[1], q2));
 }
 static double xf_scale(const ogrid *g, int k, double x, double q2)
 {
-    double xmax = g->x[g->nx - 1], qmin = g->q2[0], qmax = g->q2[g->nq_tot - 1];
+    double xmax = x_of(g, 0)[nx_of(g, 0) - 1], qmin = g->q2[0], qmax = g->q2[g->nq_tot - 1];
     if (!(x > 0.0) || !(q2 > 0.0) || !(x <= xmax) || isinf(q2)) return NAN;
     if (q2 > qmax) {
         double qa = g->q2[g->nq_tot - 2], qb = qmax;

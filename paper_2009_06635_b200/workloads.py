@@ -45,6 +45,9 @@ class PdfGridSpec:
     pids: np.ndarray  # int32
     values: np.ndarray  # flat float64
     params: dict = field(default_factory=dict)  # per-PID (A, a, b, c, d), for tests only
+    # per-sub-grid x-knot arrays (LHAPDF allows them): x_knots is then the concatenation, x_offsets
+    # (int32, n_sub + 1) delimits the sub-grids' arrays, values are [s][ix_s][iq_s][ipid]
+    x_offsets: np.ndarray = None
 
     @property
     def n_sub(self) -> int:
@@ -58,13 +61,19 @@ class PdfGridSpec:
     def n_pid(self) -> int:
         return len(self.pids)
 
+    def sub_x(self, s: int) -> np.ndarray:
+        """x knots of subgrid s."""
+        if self.x_offsets is None:
+            return self.x_knots
+        return self.x_knots[self.x_offsets[s]: self.x_offsets[s + 1]]
+
     def sub_values(self, s: int) -> np.ndarray:
         """View of subgrid s as [ix][iq][ipid]."""
         off = 0
         for r in range(s):
-            off += self.nx * int(self.q_offsets[r + 1] - self.q_offsets[r]) * self.n_pid
-        nq = int(self.q_offsets[s + 1] - self.q_offsets[s])
-        return self.values[off: off + self.nx * nq * self.n_pid].reshape(self.nx, nq, self.n_pid)
+            off += len(self.sub_x(r)) * int(self.q_offsets[r + 1] - self.q_offsets[r]) * self.n_pid
+        nq, nx = int(self.q_offsets[s + 1] - self.q_offsets[s]), len(self.sub_x(s))
+        return self.values[off: off + nx * nq * self.n_pid].reshape(nx, nq, self.n_pid)
 
     def sub_q(self, s: int) -> np.ndarray:
         return self.q_knots[self.q_offsets[s]: self.q_offsets[s + 1]]
@@ -151,6 +160,23 @@ def make_pdf_grid(x_lo, x_hi, nx, q_edges, nq_per_sub, pids, seed: int = GRID_SE
 
 NNPDF_Q_EDGES = (1.65, float(np.sqrt(1.65 * 4.92)), 4.92, 172.5, 1.0e5)
 NNPDF_NQ = (7, 14, 23, 20)
+
+
+def make_pdf_grid_xs(x_knots_per_sub, q_edges, nq_per_sub, pids, seed: int = GRID_SEED) -> PdfGridSpec:
+    """A grid whose sub-grids carry their own x-knot arrays (same first and last knot), values from the
+    analytic family on each sub-grid's own knots."""
+    params = draw_family_params(pids, seed)
+    xs = [np.asarray(x, dtype=np.float64) for x in x_knots_per_sub]
+    q_offsets, q_knots, vals = [0], [], []
+    for s, nq in enumerate(nq_per_sub):
+        q = _geomspace(q_edges[s], q_edges[s + 1], nq)
+        q_knots.append(q)
+        q_offsets.append(q_offsets[-1] + nq)
+        blk = np.stack([family_value(params[int(p)], xs[s][:, None], (q * q)[None, :]) for p in pids], axis=-1)
+        vals.append(blk.reshape(-1))
+    x_off = np.concatenate([[0], np.cumsum([len(x) for x in xs])]).astype(np.int32)
+    return PdfGridSpec(np.concatenate(xs), np.asarray(q_offsets, np.int32), np.concatenate(q_knots),
+                       np.asarray(pids, np.int32), np.concatenate(vals), params, x_offsets=x_off)
 
 
 def grid_config1() -> PdfGridSpec:
@@ -343,7 +369,8 @@ def write_lhagrid(spec: PdfGridSpec, path: str, pdf_type: str = "central", x_kno
         for s in range(spec.n_sub):
             q = spec.sub_q(s)
             if x_knots_per_sub is None:
-                xk, vals = spec.x_knots, spec.sub_values(s).reshape(spec.nx * len(q), spec.n_pid)
+                xk = spec.sub_x(s)
+                vals = spec.sub_values(s).reshape(len(xk) * len(q), spec.n_pid)
             else:
                 xk = np.asarray(x_knots_per_sub[s], dtype=np.float64)
                 vals = np.stack([family_value(spec.params[int(p)], xk[:, None], (q * q)[None, :]) for p in spec.pids], axis=-1)

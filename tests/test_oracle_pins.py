@@ -676,3 +676,46 @@ def test_lumi_helper_is_bilinear_and_symmetric():
     # the 1/(x1 x2) form, and the scale bounds the sum of term magnitudes
     assert np.allclose(oracle.lumi_events(g1, terms, x1, x2, q2, divide_by_x=True), direct / (x1 * x2), rtol=4e-16, atol=0)
     assert np.all(np.abs(direct) <= sc * (1 + 1e-12))
+
+
+# ----------------------------------------------------------------------------------
+# Per-sub-grid x-knot arrays (the LHAPDF layout allows them; "computes independently query
+# points belonging to different sub-grids"): a sub-grid with its own x knots is interpolated exactly
+# as if it were a grid of its own.
+# ----------------------------------------------------------------------------------
+def test_per_subgrid_x_knots_are_independent_grids():
+    rng = np.random.default_rng(51)
+    subs = [rand_knots(rng, 1.5, 4.0, 5), rand_knots(rng, 4.0, 30.0, 6), rand_knots(rng, 30.0, 900.0, 4)]
+    xs = [rand_knots(rng, 1e-5, 1.0, n) for n in (9, 14, 6)]
+    pids = [1, 21]
+    vals = [rng.normal(size=(len(x), len(q), len(pids))) for x, q in zip(xs, subs)]
+    x_off = np.concatenate([[0], np.cumsum([len(x) for x in xs])]).astype(np.int32)
+    q_off = np.concatenate([[0], np.cumsum([len(q) for q in subs])]).astype(np.int32)
+    og = oracle.OraclePdfGrid(np.concatenate(xs), q_off, np.concatenate(subs), pids,
+                              np.concatenate([v.reshape(-1) for v in vals]), x_offsets=x_off)
+    for s, (xk, qk, v) in enumerate(zip(xs, subs, vals)):
+        single = oracle.OraclePdfGrid(xk, [0, len(qk)], qk, pids, v.reshape(-1))
+        lo, hi = qk[0] ** 2, qk[-1] ** 2
+        n = 500
+        x = np.exp(rng.uniform(np.log(1e-7), 0.0, n))                       # in range and below x_0 (rule A)
+        x[:len(xk)] = xk
+        q2 = np.exp(rng.uniform(np.log(lo), np.log(hi), n))
+        q2 = np.clip(q2, lo, np.nextafter(hi, 0) if s + 1 < len(subs) else hi)  # the threshold itself belongs to s + 1
+        a, sa = og.xfxq2(pids, x, q2, with_scale=True)
+        b, sb = single.xfxq2(pids, x, q2, with_scale=True)
+        assert np.array_equal(a, b) and np.array_equal(sa, sb)
+    # knots of every sub-grid are reproduced exactly, thresholds in the upper sub-grid
+    for s, (xk, qk, v) in enumerate(zip(xs, subs, vals)):
+        qq = qk[:-1] if s + 1 < len(subs) else qk
+        X, Q = np.meshgrid(xk, qq ** 2, indexing="ij")
+        got = og.xfxq2(pids, X.ravel(), Q.ravel())
+        assert np.array_equal(got, v[:, :len(qq), :].transpose(2, 0, 1).reshape(len(pids), -1))
+    # one shared array passed sub-grid by sub-grid = the shared-array form, bit for bit
+    xk = xs[0]
+    vals2 = [rng.normal(size=(len(xk), len(q), len(pids))) for q in subs]
+    flat = np.concatenate([v.reshape(-1) for v in vals2])
+    shared = oracle.OraclePdfGrid(xk, q_off, np.concatenate(subs), pids, flat)
+    per = oracle.OraclePdfGrid(np.tile(xk, 3), q_off, np.concatenate(subs), pids, flat,
+                               x_offsets=np.arange(4, dtype=np.int32) * len(xk))
+    x = np.exp(rng.uniform(np.log(1e-7), 0.0, 2000)); q2 = np.exp(rng.uniform(np.log(0.5), np.log(2e6), 2000))
+    assert np.array_equal(shared.xfxq2(pids, x, q2), per.xfxq2(pids, x, q2), equal_nan=True)
