@@ -40,9 +40,9 @@ enum {
     PDFB_ECUDA = -4,    /* CUDA runtime error (no device, out of memory, launch failure) */
     PDFB_EIO = -6,      /* a file could not be opened or read                          */
     PDFB_EFORMAT = -7,  /* a file is not in the expected text layout                   */
-    PDFB_EXKNOTS = -8,  /* a well-formed member file whose sub-grids carry different x-knot
-                           arrays (or PID lists): LHAPDF allows it, this library wants one
-                           x-knot array for all sub-grids (pdf_grid_load's argument list)  */
+    PDFB_EXKNOTS = -8,  /* a well-formed member file / argument list this entry point cannot take:
+                           sub-grids with different PID lists; or sub-grids with their own x-knot
+                           arrays handed to an entry point that wants one array (use the *_xs one) */
     PDFB_ELIMIT = -5    /* more than PDFB_MAX_SUBGRIDS subgrids or PDFB_MAX_PIDS PIDs    */
 };
 #define PDFB_MAX_SUBGRIDS 16
@@ -72,6 +72,24 @@ enum {
 int pdf_grid_load(int n_sub, int nx, const double *x_knots, const int *q_offsets,
                   const double *q_knots, int n_pid, const int *pids, const double *values,
                   int device, pdfb_grid **out);
+
+/*
+ * pdf_grid_load_xs -- a member whose sub-grids carry their OWN x-knot arrays, as the LHAPDF6 grid
+ * layout allows (every sub-grid block of a member file has its own x line; the files
+ * "are directly loaded", sub-grids are interpolated independently).  The cell, the in-cell
+ * coordinate and the x derivatives of a point come from the x knots of the point's own sub-grid;
+ * below x_min the value continues from that sub-grid's first two knots.
+ *   x_offsets  host [n_sub+1], x_offsets[0] = 0; sub-grid s owns x_knots[x_offsets[s] .. x_offsets[s+1])
+ *   x_knots    host, the arrays one after the other, each strictly increasing with >= 2 knots; all
+ *              arrays must start at the same x_min and end at the same x_max (else PDFB_EKNOTS)
+ *   values     host, [s][ix_s][iq_s][ipid] with the sub-grids concatenated (file order)
+ * Other arguments as pdf_grid_load.  If the arrays are in fact identical the handle is an ordinary
+ * pdf_grid_load handle; otherwise every call on it is served by the read-only-cache kernel (correct
+ * everywhere, about an order of magnitude slower than the shared-memory kernel).
+ */
+int pdf_grid_load_xs(int n_sub, const int *x_offsets, const double *x_knots, const int *q_offsets,
+                     const double *q_knots, int n_pid, const int *pids, const double *values,
+                     int device, pdfb_grid **out);
 
 /*
  * pdf_set_load -- a PDF SET: n_members member tables on the same knots (section
@@ -232,11 +250,12 @@ long long pdfb_launch_count(void);
  *
  * Member file ("lhagrid1"): metadata header, then blocks separated by lines "---"; a block is the
  * x knots (line 1), the Q knots in GeV (line 2), the PIDs (line 3), then nx*nq lines of n_pid
- * values, x index outer, Q index inner -- pdf_grid_load's own order.  All blocks must share one
- * x-knot array and one PID list: a file whose blocks differ there is read to the end, found
- * well-formed, and refused with PDFB_EXKNOTS (distinct from PDFB_EKNOTS / PDFB_EFORMAT, so that a
- * caller can tell "valid LHAPDF file this library cannot take" from "broken file").  PDFB_EIO: cannot read; PDFB_EFORMAT: not this
- * layout.  The handle owns host memory until pdfb_lhagrid_free.
+ * values, x index outer, Q index inner -- pdf_grid_load's own order.  All blocks must share one PID
+ * list (else PDFB_EXKNOTS, after the file has been read to the end and found well-formed).  Blocks
+ * may carry different x-knot arrays: pdfb_lhagrid_dims / _get then return PDFB_EXKNOTS and
+ * pdfb_lhagrid_dims_xs / _get_xs (which serve both kinds) give pdf_grid_load_xs's arguments.
+ * PDFB_EIO: cannot read; PDFB_EFORMAT: not this layout.  The handle owns host memory until
+ * pdfb_lhagrid_free.
  *   pdfb_lhagrid_get fills caller arrays sized from pdfb_lhagrid_dims:
  *   x_knots[nx], q_offsets[n_sub+1], q_knots[nq_tot], pids[n_pid], values[nx*nq_tot*n_pid].
  */
@@ -245,6 +264,11 @@ int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out);
 int pdfb_lhagrid_dims(const pdfb_lhagrid *g, int *n_sub, int *nx, int *nq_tot, int *n_pid);
 int pdfb_lhagrid_get(const pdfb_lhagrid *g, double *x_knots, int *q_offsets, double *q_knots, int *pids,
                      double *values);
+/* x_offsets[n_sub+1], x_knots[nx_total] (the blocks' x arrays one after the other), values[n_values] */
+int pdfb_lhagrid_dims_xs(const pdfb_lhagrid *g, int *n_sub, int *nx_total, int *nq_tot, int *n_pid,
+                         long long *n_values, int *shared_x);
+int pdfb_lhagrid_get_xs(const pdfb_lhagrid *g, int *x_offsets, double *x_knots, int *q_offsets, double *q_knots,
+                        int *pids, double *values);
 void pdfb_lhagrid_free(pdfb_lhagrid *g);
 /* alpha_s nodes of a set's metadata file: the lists AlphaS_Qs (GeV, a repeated Q marks a
  * threshold) and AlphaS_Vals.  *n = node count; the arrays are filled only if cap >= *n. */

@@ -22,7 +22,7 @@ _ll = ctypes.c_longlong
 
 EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
-           "pdfb_launch_count", "pdfb_probe", "pdf_lumi_events", "pdf_xfxq2_pm", "pdf_xfxq2_f32", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
+           "pdfb_launch_count", "pdfb_probe", "pdf_lumi_events", "pdf_xfxq2_pm", "pdf_xfxq2_f32", "pdf_grid_load_xs", "pdfb_lhagrid_dims_xs", "pdfb_lhagrid_get_xs", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
            "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
 
 
@@ -189,6 +189,22 @@ def pdf_grid_load(x_knots, q_offsets, q_knots, pids, values, device: int = 0):
     return h.value
 
 
+def pdf_grid_load_xs(x_offsets, x_knots, q_offsets, q_knots, pids, values, device: int = 0):
+    """A member whose sub-grids have their own x-knot arrays (x_knots = the arrays one after the other,
+    x_offsets delimits them; values [s][ix_s][iq_s][ipid]) -> opaque handle."""
+    x_knots, q_knots, values = _f64(x_knots), _f64(q_knots), _f64(values)
+    x_offsets, q_offsets, pids = _i32(x_offsets), _i32(q_offsets), _i32(pids)
+    h = _vp()
+    L = lib()
+    L.pdf_grid_load_xs.restype = ctypes.c_int
+    L.pdf_grid_load_xs.argtypes = [ctypes.c_int, _ip, _dp, _ip, _dp, ctypes.c_int, _ip, _dp, ctypes.c_int, ctypes.POINTER(_vp)]
+    rc = L.pdf_grid_load_xs(len(q_offsets) - 1, x_offsets.ctypes.data_as(_ip), x_knots.ctypes.data_as(_dp),
+                            q_offsets.ctypes.data_as(_ip), q_knots.ctypes.data_as(_dp), len(pids),
+                            pids.ctypes.data_as(_ip), values.ctypes.data_as(_dp), int(device), ctypes.byref(h))
+    _check(rc, "pdf_grid_load_xs")
+    return h.value
+
+
 def pdf_set_load(x_knots, q_offsets, q_knots, pids, values, device: int = 0):
     """-> handle of a PDF set; values[member] = one member's table in LHAPDF grid-file order."""
     x_knots, q_knots = _f64(x_knots), _f64(q_knots)
@@ -348,6 +364,31 @@ def lhagrid_read(path: str):
     return x, off, q, pids, vals
 
 
+def lhagrid_read_xs(path: str):
+    """Parse one member file whose sub-grids may carry their own x-knot arrays ->
+    (x_offsets, x_knots, q_offsets, q_knots, pids, values, shared_x): pdf_grid_load_xs's arguments."""
+    h = _vp()
+    L = lib()
+    L.pdfb_lhagrid_dims_xs.restype = ctypes.c_int
+    L.pdfb_lhagrid_dims_xs.argtypes = [_vp] + [ctypes.POINTER(ctypes.c_int)] * 4 + [ctypes.POINTER(ctypes.c_longlong), ctypes.POINTER(ctypes.c_int)]
+    L.pdfb_lhagrid_get_xs.restype = ctypes.c_int
+    L.pdfb_lhagrid_get_xs.argtypes = [_vp, _ip, _dp, _ip, _dp, _ip, _dp]
+    _check(L.pdfb_lhagrid_read(os.fsencode(path), ctypes.byref(h)), f"pdfb_lhagrid_read({path})")
+    try:
+        d = [ctypes.c_int(0) for _ in range(4)]
+        nv, sh = ctypes.c_longlong(0), ctypes.c_int(0)
+        _check(L.pdfb_lhagrid_dims_xs(h, *[ctypes.byref(v) for v in d], ctypes.byref(nv), ctypes.byref(sh)), "pdfb_lhagrid_dims_xs")
+        n_sub, nxt, nq_tot, n_pid = (int(v.value) for v in d)
+        x, q = np.empty(nxt), np.empty(nq_tot)
+        xoff, off, pids = np.empty(n_sub + 1, np.int32), np.empty(n_sub + 1, np.int32), np.empty(n_pid, np.int32)
+        vals = np.empty(int(nv.value))
+        _check(L.pdfb_lhagrid_get_xs(h, xoff.ctypes.data_as(_ip), x.ctypes.data_as(_dp), off.ctypes.data_as(_ip),
+                                     q.ctypes.data_as(_dp), pids.ctypes.data_as(_ip), vals.ctypes.data_as(_dp)), "pdfb_lhagrid_get_xs")
+    finally:
+        L.pdfb_lhagrid_free(h)
+    return xoff, x, off, q, pids, vals, bool(sh.value)
+
+
 def lhapdf_info_alphas(info_path: str):
     """-> (q_knots, alphas) of a set's metadata file."""
     n = ctypes.c_int(0)
@@ -372,6 +413,14 @@ def load_lhapdf_set(set_dir: str, members=None, device: int = 0):
     if members is None:
         members = range(lhapdf_info_members(info))
     first, tables = None, []
+    members = list(members)
+    xs = lhagrid_read_xs(os.path.join(set_dir, f"{name}_{int(members[0]):04d}.dat"))
+    if not xs[6]:  # sub-grids with their own x-knot arrays: one member, read-only-cache kernel
+        if len(members) != 1:
+            raise PdfbError(PDFB_EXKNOTS, f"{name}: sets whose sub-grids carry their own x-knot arrays load one member at a time")
+        hp = pdf_grid_load_xs(xs[0], xs[1], xs[2], xs[3], xs[4], xs[5], device)
+        qa, aa = lhapdf_info_alphas(info)
+        return hp, alphas_grid_load(qa, aa, device), xs[4]
     for m in members:
         x, off, q, pids, vals = lhagrid_read(os.path.join(set_dir, f"{name}_{int(m):04d}.dat"))
         if first is None:
@@ -387,6 +436,8 @@ def load_lhapdf_set(set_dir: str, members=None, device: int = 0):
 
 # ------------------------------------------------------------------ spec conveniences
 def load_pdf_spec(spec, device: int = 0):
+    if getattr(spec, "x_offsets", None) is not None:
+        return pdf_grid_load_xs(spec.x_offsets, spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, spec.values, device)
     return pdf_grid_load(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, spec.values, device)
 
 

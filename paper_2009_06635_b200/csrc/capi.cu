@@ -23,7 +23,7 @@ extern "C" const char *pdfb_strerror(int code)
     case PDFB_ECUDA: return "CUDA runtime error (no device, out of memory or launch failure)";
     case PDFB_EIO: return "file could not be opened or read";
     case PDFB_EFORMAT: return "file is not in the expected LHAPDF text layout";
-    case PDFB_EXKNOTS: return "sub-grids with different x-knot arrays or PID lists are not supported (one x-knot array for all sub-grids)";
+    case PDFB_EXKNOTS: return "sub-grids with different PID lists, or sub-grids with their own x-knot arrays passed to an entry point that takes one array (use pdf_grid_load_xs / pdfb_lhagrid_*_xs)";
     case PDFB_ELIMIT: return "too many sub-grids, PIDs or alpha_s nodes";
     default: return "unknown pdfb error code";
     }

@@ -17,9 +17,10 @@
 #include "pdfb_internal.cuh"
 
 struct pdfb_lhagrid {
-    int n_sub = 0, nx = 0, n_pid = 0;
-    std::vector<double> x, q, values;  // q and values concatenated over the blocks
-    std::vector<int> q_off, pids;
+    int n_sub = 0, nx = 0, n_pid = 0;  // nx: knots of the first block's x array
+    bool shared_x = true;              // every block carries the same x-knot array
+    std::vector<double> x, q, values;  // x: the blocks' x arrays, q and values: concatenated over the blocks
+    std::vector<int> x_off, q_off, pids;
 };
 
 static bool read_all(const char *path, std::string &s)
@@ -82,7 +83,8 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
     ++i;
     std::vector<double> row, xk, qk;
     int rc = PDFB_OK;
-    bool mixed_x = false;  // blocks with different x knots / PIDs: parsed to the end, then refused as such
+    bool mixed_pids = false;  // blocks with different PID lists: parsed to the end, then refused as such
+    std::vector<double> x0;
     g->q_off.push_back(0);
     while (i < lines.size() && !rc) {
         while (i < lines.size() && is_blank(lines[i])) ++i;
@@ -95,15 +97,19 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
         std::vector<int> pids(row.size());
         for (size_t k = 0; k < row.size(); k++) pids[k] = (int)row[k];
         if (g->n_sub == 0) {
-            g->x = xk; g->nx = (int)xk.size(); g->pids = pids; g->n_pid = (int)pids.size();
-        } else if (xk != g->x || pids != g->pids) {
-            mixed_x = true;  // this library wants one x-knot array and one PID list for all sub-grids
+            x0 = xk; g->nx = (int)xk.size(); g->pids = pids; g->n_pid = (int)pids.size();
+            g->x_off.push_back(0);
+        } else {
+            if (pids != g->pids) mixed_pids = true;  // one PID list for all sub-grids
+            if (xk != x0) g->shared_x = false;       // own x knots per sub-grid: pdf_grid_load_xs
         }
+        g->x.insert(g->x.end(), xk.begin(), xk.end());
+        g->x_off.push_back((int)g->x.size());
         const size_t nrows = xk.size() * qk.size();
         for (size_t r = 0; r < nrows && !rc; r++, i++) {
             if (i >= lines.size() || is_sep(lines[i]) || !parse_doubles(lines[i].first, lines[i].second, row) ||
                 row.size() != pids.size()) { rc = PDFB_EFORMAT; break; }
-            if (!mixed_x) g->values.insert(g->values.end(), row.begin(), row.end());
+            if (!mixed_pids) g->values.insert(g->values.end(), row.begin(), row.end());
         }
         if (rc) break;
         g->q.insert(g->q.end(), qk.begin(), qk.end());
@@ -116,7 +122,7 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
         }
     }
     if (!rc && g->n_sub == 0) rc = PDFB_EFORMAT;
-    if (!rc && mixed_x) rc = PDFB_EXKNOTS;
+    if (!rc && mixed_pids) rc = PDFB_EXKNOTS;
     if (!rc && g->n_sub > PDFB_MAX_SUBGRIDS) rc = PDFB_ELIMIT;
     if (rc) { delete g; return rc; }
     *out = g;
@@ -126,6 +132,7 @@ extern "C" int pdfb_lhagrid_read(const char *path, pdfb_lhagrid **out)
 extern "C" int pdfb_lhagrid_dims(const pdfb_lhagrid *g, int *n_sub, int *nx, int *nq_tot, int *n_pid)
 {
     if (!g || !n_sub || !nx || !nq_tot || !n_pid) return PDFB_EINVAL;
+    if (!g->shared_x) return PDFB_EXKNOTS;  // own x knots per sub-grid: pdfb_lhagrid_dims_xs / _get_xs
     *n_sub = g->n_sub; *nx = g->nx; *nq_tot = (int)g->q.size(); *n_pid = g->n_pid;
     return PDFB_OK;
 }
@@ -134,6 +141,29 @@ extern "C" int pdfb_lhagrid_get(const pdfb_lhagrid *g, double *x_knots, int *q_o
                                 double *values)
 {
     if (!g || !x_knots || !q_offsets || !q_knots || !pids || !values) return PDFB_EINVAL;
+    if (!g->shared_x) return PDFB_EXKNOTS;
+    memcpy(x_knots, g->x.data(), sizeof(double) * g->nx);
+    memcpy(q_offsets, g->q_off.data(), sizeof(int) * g->q_off.size());
+    memcpy(q_knots, g->q.data(), sizeof(double) * g->q.size());
+    memcpy(pids, g->pids.data(), sizeof(int) * g->pids.size());
+    memcpy(values, g->values.data(), sizeof(double) * g->values.size());
+    return PDFB_OK;
+}
+
+extern "C" int pdfb_lhagrid_dims_xs(const pdfb_lhagrid *g, int *n_sub, int *nx_total, int *nq_tot, int *n_pid,
+                                    long long *n_values, int *shared_x)
+{
+    if (!g || !n_sub || !nx_total || !nq_tot || !n_pid || !n_values || !shared_x) return PDFB_EINVAL;
+    *n_sub = g->n_sub; *nx_total = (int)g->x.size(); *nq_tot = (int)g->q.size(); *n_pid = g->n_pid;
+    *n_values = (long long)g->values.size(); *shared_x = g->shared_x ? 1 : 0;
+    return PDFB_OK;
+}
+
+extern "C" int pdfb_lhagrid_get_xs(const pdfb_lhagrid *g, int *x_offsets, double *x_knots, int *q_offsets, double *q_knots,
+                                   int *pids, double *values)
+{
+    if (!g || !x_offsets || !x_knots || !q_offsets || !q_knots || !pids || !values) return PDFB_EINVAL;
+    memcpy(x_offsets, g->x_off.data(), sizeof(int) * g->x_off.size());
     memcpy(x_knots, g->x.data(), sizeof(double) * g->x.size());
     memcpy(q_offsets, g->q_off.data(), sizeof(int) * g->q_off.size());
     memcpy(q_knots, g->q.data(), sizeof(double) * g->q.size());

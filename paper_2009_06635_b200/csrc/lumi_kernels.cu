@@ -233,7 +233,7 @@ k_lumi_band(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef 
 // Events the band kernel does not take: a point outside the grid, a coordinate without a value, or a
 // grid without the shared-memory path (all == 1: every event).  One thread per event.
 __global__ void __launch_bounds__(128, 8)  // few registers: the usual case is a scan that finds nothing to do
-k_lumi_general(GridDev g, const __grid_constant__ LumiCoef C, int nf, int all, long long n, const double *__restrict__ x1,
+k_lumi_general(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef C, int nf, int all, long long n, const double *__restrict__ x1,
                const double *__restrict__ x2, const double *__restrict__ q2, double *__restrict__ out, int flags)
 {
     const long long e = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -244,14 +244,17 @@ k_lumi_general(GridDev g, const __grid_constant__ LumiCoef C, int nf, int all, l
     ReqCols rc;
     rc.n = nf;
     for (int k = 0; k < nf; k++) rc.col[k] = k;
-    double f1[PDFB_LUMI_MAXF], f2[PDFB_LUMI_MAXF];
-    const bool ok1 = xf_point_v0(g, g.val, rc, xa, qv, f1), ok2 = xf_point_v0(g, g.val, rc, xb, qv, f2);
-    double lum = 0.0;
+    // beam 2 first: hv[a] = sum_b c[a][b] xf_b(x2); then beam 1 into the same array and the sum over a
+    double f[PDFB_LUMI_MAXF], hv[PDFB_LUMI_MAXF];
+    const bool ok2 = xf_point_v0(g, g.val, rc, xb, qv, f);
     for (int a = 0; a < nf; a++) {
         double h = 0.0;
-        for (int b = 0; b < nf; b++) h = fma(C.c[a][b], f2[b], h);
-        lum = fma(f1[a], h, lum);
+        for (int b = 0; b < nf; b++) h = fma(C.c[a][b], f[b], h);
+        hv[a] = h;
     }
+    const bool ok1 = xf_point_v0(g, g.val, rc, xa, qv, f);
+    double lum = 0.0;
+    for (int a = 0; a < nf; a++) lum = fma(f[a], hv[a], lum);
     if (flags & 1) lum /= xa * xb;
     if (!ok1 || !ok2) {
         lum = __longlong_as_double(0x7ff8000000000000LL);

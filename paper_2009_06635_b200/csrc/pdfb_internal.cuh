@@ -144,6 +144,11 @@ struct GridDev {
     double Va, Vb, inv_dVab;           // ln of the last two Q^2 knots, 1/(Vb-Va)
     int jC;                            // interval of 1.01*q2_min in sub-grid 0
     double wvC[4];                     // its four v weights (fixed per grid), stencil order j-1..j+2
+    // sub-grids with their own x-knot arrays (pdf_grid_load_xs; read-only-cache kernel only): sub-grid s owns
+    // xk / xrec [x_off[s], x_off[s+1]); rule A continues from its first two knots: U0, inv_dU01s[s]
+    int xs_per_sub;
+    int x_off[PDFB_MAX_SUBGRIDS + 1];
+    double inv_dU01s[PDFB_MAX_SUBGRIDS];
     const double *xk;                  // [nx] x knots
     const double *q2k;                 // [nq_tot] Q^2 knots
     const IntervalRec *xrec;           // [nx-1]

@@ -89,37 +89,41 @@ __device__ __forceinline__ bool xf_point_v0(const GridDev &g, const double *__re
     }
     const bool low_x = xv < g.x_min, high_q = qv > g.q2_max, low_q = qv < g.q2_min;
 
+    // ---- sub-grid of the point (O3 step 1; the Q^2 rules probe the last / the first sub-grid)
+    int s = 0;
+    if (high_q) s = g.n_sub - 1;
+    else if (!low_q)
+        for (int r = 1; r < g.n_sub; r++) if (g.q2_lo[r] <= qv) s = r;
+    const int nq = g.q_off[s + 1] - g.q_off[s];
+    // its x knots: one array for all sub-grids, or its own (pdf_grid_load_xs)
+    const int xo = g.xs_per_sub ? g.x_off[s] : 0, nxs = g.xs_per_sub ? g.x_off[s + 1] - g.x_off[s] : g.nx;
+
     // ---- u direction: one set (in range) or the two one-hot sets of knots 0 and 1 (rule A)
     Set4 u1, u2;
     double rA = 0.0;
     if (!low_x) {
-        int i = find_interval(g.xk, g.nx, xv);
-        IntervalRec r = load_rec(g.xrec + i);
+        int i = find_interval(g.xk + xo, nxs, xv);
+        IntervalRec r = load_rec(g.xrec + xo + i);
         double w[4];
         weights4(r, (pdfb_ln(xv) - r.z0) * r.inv_dz, w);
-        u1 = make_set(i, g.nx, w);
+        u1 = make_set(i, nxs, w);
     } else {
-        rA = (pdfb_ln(xv) - g.U0) * g.inv_dU01;
+        rA = (pdfb_ln(xv) - g.U0) * (g.xs_per_sub ? g.inv_dU01s[s] : g.inv_dU01);
         u1.base = 0; u1.w[0] = 1.0; u1.w[1] = u1.w[2] = u1.w[3] = 0.0;
         u2.base = 0; u2.w[1] = 1.0; u2.w[0] = u2.w[2] = u2.w[3] = 0.0;
     }
     // ---- v direction: one set (in range), or two sets (rules B, C)
     Set4 v1, v2;
-    int s = 0, nq;
     double rB = 0.0;
     if (high_q) {  // probes at the last two Q^2 knots of the last sub-grid
-        s = g.n_sub - 1; nq = g.q_off[s + 1] - g.q_off[s];
         rB = (pdfb_ln(qv) - g.Va) * g.inv_dVab;
         int base = max(nq - 4, 0), ia = nq - 2 - base, ib = nq - 1 - base;
         v1.base = v2.base = base;
         for (int b = 0; b < 4; b++) { v1.w[b] = (b == ia) ? 1.0 : 0.0; v2.w[b] = (b == ib) ? 1.0 : 0.0; }
     } else if (low_q) {  // probes at q_min (knot 0 of sub-grid 0) and at 1.01 q_min
-        s = 0; nq = g.q_off[1];
         v1.base = 0; v1.w[0] = 1.0; v1.w[1] = v1.w[2] = v1.w[3] = 0.0;
         v2 = make_set(g.jC, nq, g.wvC);
     } else {
-        for (int r = 1; r < g.n_sub; r++) if (g.q2_lo[r] <= qv) s = r;
-        nq = g.q_off[s + 1] - g.q_off[s];
         int j = find_interval(g.q2k + g.q_off[s], nq, qv);
         IntervalRec r = load_rec(g.qrec + g.q_off[s] + j);
         double w[4];
@@ -134,14 +138,14 @@ __device__ __forceinline__ bool xf_point_v0(const GridDev &g, const double *__re
         int col = rc.col[r];
         double y1, y2 = 0.0;
         if (!low_x) {
-            y1 = contract(val, g.kpad, g.nx, voff, u1, v1, nq, col);
-            if (two_v) y2 = contract(val, g.kpad, g.nx, voff, u1, v2, nq, col);
+            y1 = contract(val, g.kpad, nxs, voff, u1, v1, nq, col);
+            if (two_v) y2 = contract(val, g.kpad, nxs, voff, u1, v2, nq, col);
         } else {  // rule A applied to each v probe
-            y1 = continuation(rA, contract(val, g.kpad, g.nx, voff, u1, v1, nq, col),
-                              contract(val, g.kpad, g.nx, voff, u2, v1, nq, col));
+            y1 = continuation(rA, contract(val, g.kpad, nxs, voff, u1, v1, nq, col),
+                              contract(val, g.kpad, nxs, voff, u2, v1, nq, col));
             if (two_v)
-                y2 = continuation(rA, contract(val, g.kpad, g.nx, voff, u1, v2, nq, col),
-                                  contract(val, g.kpad, g.nx, voff, u2, v2, nq, col));
+                y2 = continuation(rA, contract(val, g.kpad, nxs, voff, u1, v2, nq, col),
+                                  contract(val, g.kpad, nxs, voff, u2, v2, nq, col));
         }
         double out = y1;
         if (high_q) {

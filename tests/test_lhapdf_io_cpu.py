@@ -80,18 +80,33 @@ def test_missing_file_and_mismatched_blocks(tmp_path):
     blocks[2] = "\n".join(lines)
     (tmp_path / "bad.dat").write_text("---\n".join(blocks))
     with pytest.raises(B.PdfbError) as e:
-        B.lhagrid_read(str(tmp_path / "bad.dat"))
+        B.lhagrid_read(str(tmp_path / "bad.dat"))      # the one-x-array reader says which API takes the file
     assert e.value.code == B.PDFB_EXKNOTS
-    # a complete, well-formed member file whose sub-grids have x-knot arrays of different LENGTHS (as
-    # LHAPDF allows): read to the end and refused with the distinct code, not as a malformed file
-    xs = [spec.x_knots, W._geomspace(1e-9, 1.0, 80), spec.x_knots[::2].copy(), W._geomspace(1e-9, 1.0, 120)]
-    W.write_lhagrid(spec, str(tmp_path / "perx.dat"), x_knots_per_sub=xs)
+    assert not B.lhagrid_read_xs(str(tmp_path / "bad.dat"))[6]
+    # a member file whose sub-grids have x-knot arrays of different LENGTHS (as LHAPDF allows) round-trips
+    # through the *_xs reader into pdf_grid_load_xs's arguments
+    xs = [spec.x_knots, W._geomspace(1e-9, 1.0, 80), spec.x_knots[::3].copy(), W._geomspace(1e-9, 1.0, 120)]
+    sx = W.make_pdf_grid_xs(xs, (1.65, (1.65 * 4.92) ** 0.5, 4.92, 172.5, 1.0e5), (7, 14, 23, 20), W.PIDS_11)
+    W.write_lhagrid(sx, str(tmp_path / "perx.dat"))
+    xoff, x, qoff, q, pids, vals, shared = B.lhagrid_read_xs(str(tmp_path / "perx.dat"))
+    assert not shared and np.array_equal(xoff, sx.x_offsets) and np.array_equal(x, sx.x_knots)
+    assert np.array_equal(qoff, sx.q_offsets) and np.array_equal(q, sx.q_knots) and np.array_equal(vals, sx.values)
+    # a shared-x file through the same reader
+    W.write_lhagrid(spec, str(tmp_path / "shared.dat"))
+    r = B.lhagrid_read_xs(str(tmp_path / "shared.dat"))
+    assert r[6] and np.array_equal(r[1], np.tile(spec.x_knots, spec.n_sub)) and np.array_equal(r[5], spec.values)
+    # sub-grids with different PID lists: well-formed, refused with the distinct code
+    blocks = (tmp_path / "perx.dat").read_text().split("---\n")
+    lines = blocks[2].split("\n")
+    lines[2] = lines[2].replace("21", "22")
+    blocks[2] = "\n".join(lines)
+    (tmp_path / "pids.dat").write_text("---\n".join(blocks))
     with pytest.raises(B.PdfbError) as e:
-        B.lhagrid_read(str(tmp_path / "perx.dat"))
-    assert e.value.code == B.PDFB_EXKNOTS and "x-knot" in str(e.value)
-    # ... while the same file cut short is still a malformed file
+        B.lhagrid_read_xs(str(tmp_path / "pids.dat"))
+    assert e.value.code == B.PDFB_EXKNOTS
+    # ... while a file cut short is a malformed file
     txt = (tmp_path / "perx.dat").read_text().split("\n")
     (tmp_path / "perx_cut.dat").write_text("\n".join(txt[: len(txt) // 2]) + "\n")
     with pytest.raises(B.PdfbError) as e:
-        B.lhagrid_read(str(tmp_path / "perx_cut.dat"))
+        B.lhagrid_read_xs(str(tmp_path / "perx_cut.dat"))
     assert e.value.code == B.PDFB_EFORMAT

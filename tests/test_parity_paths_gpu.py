@@ -209,3 +209,77 @@ def test_point_major_and_fp32_output(torch_cuda, grid2, ograph2, monkeypatch, fo
         half_ulp32 = 0.5 * np.spacing(np.abs(ref[ok]).astype(np.float32)).astype(np.float64)
         assert np.all(np.abs(got32[ok] - ref[ok]) <= half_ulp32 + 1e-12 * np.abs(ref[ok]) + 1e-15 + 1e-12 * sc[ok])
     B.pdf_grid_free(h)
+
+
+def test_per_subgrid_x_knot_arrays(torch_cuda, tmp_path):
+    """pdf_grid_load_xs ("allowing per-subgrid x-knot arrays"): sub-grids
+    with 100 / 80 / 34 / 120 x knots on one Q^2 layout, loaded directly and from a member file in the
+    LHAPDF text layout; every knot of every sub-grid exactly, random points in and outside the grid,
+    pdf_lumi_events, the Q entry point and the output variants; identical arrays give an ordinary handle."""
+    torch = torch_cuda
+    base = W.grid_nnpdf_shaped()
+    xs = [base.x_knots, W._geomspace(1e-9, 1.0, 80), base.x_knots[::3].copy(), W._geomspace(1e-9, 1.0, 120)]
+    spec = W.make_pdf_grid_xs(xs, (1.65, (1.65 * 4.92) ** 0.5, 4.92, 172.5, 1.0e5), (7, 14, 23, 20), W.PIDS_11)
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    h = B.load_pdf_spec(spec)
+    assert not B.pdf_grid_uses_smem_path(h)
+    pids = list(W.PIDS_11)
+
+    def run(x, q2, req=pids):
+        out = torch.empty((len(req), len(x)), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h, req, torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), out)
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+    for s in range(spec.n_sub):   # knots reproduced bit for bit; a threshold belongs to the upper sub-grid
+        q = spec.sub_q(s) if s + 1 == spec.n_sub else spec.sub_q(s)[:-1]
+        X, Q = np.meshgrid(spec.sub_x(s), q ** 2, indexing="ij")
+        ref = spec.sub_values(s)[:, :len(q), :].transpose(2, 0, 1).reshape(len(pids), -1)
+        got = run(X.ravel().copy(), Q.ravel().copy())
+        inner = (X.ravel() < 1.0)   # t = 0 exactly at a knot; at x_max t = (u - U)(1/dU) is 1 to an ulp only
+        assert np.array_equal(got[:, inner], ref[:, inner])
+        check_parity(got, ref, what="per-sub-grid x knots, knots")
+    x, q2 = W.queries_extrapolation_mix(base, 150_011)
+    ref, sc = og.xfxq2(pids, x, q2, with_scale=True)
+    st = check_parity(run(x, q2), ref, sc, max_clause_frac=5e-3, what="per-sub-grid x knots, mix")
+    print(st)
+    sub = [21, -3, 0]
+    rs, ss = og.xfxq2(sub, x, q2, with_scale=True)
+    check_parity(run(x, q2, sub), rs, ss, max_clause_frac=5e-3, what="per-sub-grid x knots, PID subset")
+    # the fused call goes through the general kernel on such a grid
+    n = 40_001
+    x1, x2, qe = W.queries_mc_events(base, n)
+    terms = [(1, -1, 1.0), (-2, 2, 0.5), (21, 21, 0.25), (21, 3, -1.0)]
+    lum = torch.empty(n, dtype=torch.float64, device="cuda")
+    B.pdf_lumi_events(h, terms, torch.from_numpy(x1).cuda(), torch.from_numpy(x2).cuda(), torch.from_numpy(qe).cuda(), lum)
+    torch.cuda.synchronize()
+    lr, ls = oracle.lumi_events(og, terms, x1, x2, qe, with_scale=True)
+    check_parity(lum.cpu().numpy(), lr, ls, what="per-sub-grid x knots, lumi")
+    # the same member through a file in the LHAPDF text layout
+    d = tmp_path / "xsset"
+    d.mkdir()
+    W.write_lhagrid(spec, str(d / "xsset_0000.dat"))
+    W.write_lhapdf_info(str(d / "xsset.info"), 1, pids, W.make_alphas_grid())
+    hf, ha, fp = B.load_lhapdf_set(str(d))
+    o1 = torch.empty((len(pids), len(x)), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(hf, pids, torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), o1)
+    torch.cuda.synchronize()
+    assert np.array_equal(o1.cpu().numpy(), run(x, q2), equal_nan=True) and list(fp) == pids
+    B.pdf_grid_free(hf); B.alphas_grid_free(ha); B.pdf_grid_free(h)
+    # identical arrays passed per sub-grid: an ordinary (shared-memory) handle, same numbers as pdf_grid_load
+    same = B.pdf_grid_load_xs(np.arange(5, dtype=np.int32) * base.nx, np.tile(base.x_knots, 4), base.q_offsets,
+                              base.q_knots, base.pids, base.values)
+    plain = B.load_pdf_spec(base)
+    assert B.pdf_grid_uses_smem_path(same)
+    a = torch.empty((len(pids), len(x)), dtype=torch.float64, device="cuda"); b = torch.empty_like(a)
+    B.pdf_xfxq2(same, pids, torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), a)
+    B.pdf_xfxq2(plain, pids, torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), b)
+    torch.cuda.synchronize()
+    assert torch.equal(torch.nan_to_num(a, nan=-9.0), torch.nan_to_num(b, nan=-9.0))
+    B.pdf_grid_free(same); B.pdf_grid_free(plain)
+    # arrays that do not span one common x range are refused
+    bad = [base.x_knots, W._geomspace(1e-8, 1.0, 80), base.x_knots, base.x_knots]
+    sb = W.make_pdf_grid_xs(bad, (1.65, (1.65 * 4.92) ** 0.5, 4.92, 172.5, 1.0e5), (7, 14, 23, 20), W.PIDS_11)
+    with pytest.raises(B.PdfbError) as e:
+        B.load_pdf_spec(sb)
+    assert e.value.code == B.PDFB_EKNOTS
