@@ -92,7 +92,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
 
     pdfb_grid *g = new (std::nothrow) pdfb_grid();
     if (!g) return PDFB_EINVAL;
-    memset(g, 0, sizeof(*g));
+    g->rr_next.store(0);  // (new pdfb_grid() value-initialises: every other member is zero)
     g->device = device;
     if (cudaDeviceGetAttribute(&g->sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { delete g; return PDFB_ECUDA; }
     GridDev &d = g->d;

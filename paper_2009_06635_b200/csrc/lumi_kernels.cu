@@ -29,7 +29,8 @@
 #define LUMI_NT 512
 #define LUMI_LIST 64  // entries per warp list
 
-struct LumiCoef { double c[PDFB_LUMI_MAXF][PDFB_LUMI_MAXF]; };
+// c[a][b]; need1 / need2: bit p set if beam 1 / beam 2 needs a column of pair p (a pair no term refers to is not gathered)
+struct LumiCoef { double c[PDFB_LUMI_MAXF][PDFB_LUMI_MAXF]; unsigned need1, need2; };
 
 // the sixteen products (x weight of the knot read at step s) x (v weight of its row), for one beam
 struct Beam { uint32_t a[8]; double w[2][8]; };
@@ -162,6 +163,7 @@ k_lumi_band(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef 
                 for (int b = 0; b < NF; b++) h[b] = 0.0;
 #pragma unroll
                 for (int p = 0; p < NPAIR; p++) {
+                    if (!((C.need1 >> p) & 1)) continue;  // uniform: no term takes a flavour of this pair from beam 1
                     double f0, f1;
                     pair_value(bm, (uint32_t)(p * L.pair_stride), 2u * RB, f0, f1);
 #pragma unroll
@@ -179,6 +181,7 @@ k_lumi_band(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef 
                 make_beam(bm, row0, RB, i - 1, wu, vw, lane8);
 #pragma unroll
                 for (int p = 0; p < NPAIR; p++) {
+                    if (!((C.need2 >> p) & 1)) continue;
                     double f0, f1;
                     pair_value(bm, (uint32_t)(p * L.pair_stride), 2u * RB, f0, f1);
                     lum = fma(h[2 * p + 1], f1, fma(h[2 * p], f0, lum));
@@ -325,6 +328,7 @@ extern "C" int pdf_lumi_events(const pdfb_grid *g, const pdfb_alphas *a, int n_t
         if (ca < 0 || cb < 0) return PDFB_EPID;
         if (!std::isfinite(coeff[t])) return PDFB_EINVAL;
         C.c[ca][cb] += coeff[t];
+        C.need1 |= 1u << (ca >> 1); C.need2 |= 1u << (cb >> 1);
     }
     if (n == 0) return PDFB_OK;
     DeviceGuard guard(g->device);
