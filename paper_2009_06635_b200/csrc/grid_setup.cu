@@ -144,33 +144,36 @@ int pdfb_setup_group_slices(const double *d_src, double *d_valg, int s_knot_off,
     return PDFB_OK;
 }
 
-// alpha_s fast-path records: cubic coefficients of each interval in t, from the O2 records.
-// p(t) = h00 y0 + h10 dL + h01 y1 + h11 dH = y0 + dL t + (3(y1-y0) - 2 dL - dH) t^2 + (dL + dH - 2(y1-y0)) t^3
+// alpha_s fast-path records: cubic coefficients of each interval in s = ln Q^2 - Z_m, from the O2 records.
+// p(t) = h00 y0 + h10 dL + h01 y1 + h11 dH = y0 + dL t + (3(y1-y0) - 2 dL - dH) t^2 + (dL + dH - 2(y1-y0)) t^3,
+// t = s / dZ: alpha_s(s) = d0 + s (d1 + s (d2 + s d3)) with d_k = c_k / dZ^k -- five doubles per interval,
+// {Z_m, d0 | d1, d2} as two 128-byte lines of 8 copies (LDS.128, lane l reads copy l & 7) and d3 as one line of
+// 16 copies (LDS.64, copy l & 15): 10 conflict-free wavefronts per warp (c0..c3 + {Z, 1/dZ}: 12).
 // (the fast path takes its logarithms with ln_tab, pdfb_internal.cuh: the node logarithm stored here
-// comes from the same function, so that a query on a node gets t = 0 exactly)
+// comes from the same function, so that a query on a node gets s = 0 exactly and returns the node value)
 __global__ void k1_alphas_lines(const IntervalRec *__restrict__ rec, const double *__restrict__ a,
                                 const double *__restrict__ q2k, unsigned char *__restrict__ lines,
                                 const double2 *__restrict__ lntab, int lo, int M)
 {
     int m = blockIdx.x * blockDim.x + threadIdx.x;  // interval m of the sub-grid [lo, lo+M)
     if (m >= M) return;
-    double chunk[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    double d[4] = {0.0, 0.0, 0.0, 0.0};
     const IntervalRec r = rec[lo + m];
     const double q = q2k[lo + m];
-    chunk[0][0] = ln_tab(q, lntab[ln_tab_bin(q) * 8]); chunk[0][1] = r.inv_dz;
+    const double z = ln_tab(q, lntab[ln_tab_bin(q) * 8]);
     if (m < M - 1) {
         const double y0 = a[lo + m], y1 = a[lo + m + 1];
         const double ym = a[lo + max(m - 1, 0)], yp = a[lo + min(m + 2, M - 1)];
         const double dL = fma(r.aLm, ym, fma(r.aL0, y0, r.aL1 * y1));
         const double dH = fma(r.aHp, yp, fma(r.aH0, y0, r.aH1 * y1));
         const double dy = y1 - y0;
-        chunk[1][0] = y0; chunk[1][1] = dL;
-        chunk[2][0] = 3.0 * dy - 2.0 * dL - dH;
-        chunk[2][1] = dL + dH - 2.0 * dy;
+        d[0] = y0;
+        d[1] = dL * r.inv_dz;
+        d[2] = (3.0 * dy - 2.0 * dL - dH) * r.inv_dz * r.inv_dz;
+        d[3] = (dL + dH - 2.0 * dy) * r.inv_dz * r.inv_dz * r.inv_dz;
     }
     double2 *dst = reinterpret_cast<double2 *>(lines + (size_t)(lo + m) * PDFB_ALPHAS_LINE);
-    for (int k = 0; k < 3; k++)
-        for (int c = 0; c < 8; c++) dst[k * 8 + c] = make_double2(chunk[k][0], chunk[k][1]);
+    for (int c = 0; c < 8; c++) { dst[c] = make_double2(z, d[0]); dst[8 + c] = make_double2(d[1], d[2]); dst[16 + c] = make_double2(d[3], d[3]); }
 }
 
 int pdfb_setup_alphas_fast(const IntervalRec *d_rec, const double *d_a, const double *d_q2k, unsigned char *d_lines,

@@ -210,9 +210,9 @@ struct AlphasDev {
     const double *q2k;        // [K]
     const double *a;          // [K]
     const IntervalRec *rec;   // [K]
-    // fast path (alphas_kernels.cu): per interval 3 lines of 128 B; line k = the 16-byte chunk k of
-    // {ln knot, 1/d | c0, c1 | c2, c3} repeated 8 times, so lane l reads slot (l & 7) of each
-    // line: conflict-free whatever intervals the lanes want.  alpha_s(t) = c0 + t(c1 + t(c2 + t c3)).
+    // fast path (alphas_kernels.cu): per interval 3 lines of 128 B: {ln knot Z, d0} x 8, {d1, d2} x 8, d3 x 16,
+    // so lane l reads copy (l & 7) of the first two (LDS.128) and copy (l & 15) of the third (LDS.64):
+    // conflict-free whatever intervals the lanes want.  alpha_s = d0 + s(d1 + s(d2 + s d3)), s = ln Q^2 - Z.
     int fast_ok;
     const unsigned char *fast;  // [lines: K*384 B][ln table: PDFB_LNTAB_BYTES][q2k: K doubles][lut: PDFB_LUT_BINS u16]
     int fast_bytes, f_lntab, f_q2k, f_lut;

@@ -1,0 +1,127 @@
+"""GPU checks of what DESIGN.md promises about a handle in use, beyond element-wise parity:
+several streams evaluating on ONE handle at the same time (the per-SM scratch of the out-of-grid
+class lists, the row-range slots of small batches), bit-identical results run to run, and batch
+sizes around every granularity of the launch (a warp, a tile, the row-range threshold)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from paper_2009_06635_b200 import binding as B, build, workloads as W
+from parity_util import check_parity
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    build.build()
+    B.lib()
+    return torch
+
+
+@pytest.fixture(scope="module")
+def h2(torch_cuda, grid2):
+    h = B.load_pdf_spec(grid2)
+    yield h
+    B.pdf_grid_free(h)
+
+
+def test_streams_share_one_handle(torch_cuda, grid2, ograph2, h2):
+    """Four streams, each with its own extrapolation-mix batch (30 % of the points go through the
+    class lists in the handle's scratch), all in flight on one handle, several rounds: every result
+    equals the one the same batch gives alone, bit for bit, and agrees with the oracle."""
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    n = 400_003
+    batches = []
+    for k in range(4):
+        x, q2 = W.queries_extrapolation_mix(grid2, n, config=7000 + k)
+        batches.append((torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), x, q2))
+    alone = []
+    for dx, dq, _, _ in batches:
+        out = torch.empty((len(pids), n), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h2, pids, dx, dq, out)
+        torch.cuda.synchronize()
+        alone.append(out)
+    streams = [torch.cuda.Stream() for _ in batches]
+    outs = [torch.empty((len(pids), n), dtype=torch.float64, device="cuda") for _ in batches]
+    for rnd in range(5):
+        for o in outs:
+            o.fill_(float("nan"))
+        torch.cuda.synchronize()
+        for (dx, dq, _, _), s, o in zip(batches, streams, outs):
+            B.pdf_xfxq2(h2, pids, dx, dq, o, stream=s)
+        torch.cuda.synchronize()
+        for k, (o, a) in enumerate(zip(outs, alone)):
+            assert torch.equal(o.view(torch.int64), a.view(torch.int64)), (rnd, k)
+    _, _, x, q2 = batches[0]
+    ref, sc = ograph2.xfxq2(pids, x[:50_000], q2[:50_000], with_scale=True)
+    check_parity(alone[0][:, :50_000].cpu().numpy(), ref, sc, max_clause_frac=5e-3, what="streams")
+    assert B.pdf_grid_status(h2) == 0
+
+
+def test_small_batches_in_flight_share_the_row_range_slots(torch_cuda, grid2, ograph2, h2):
+    """Small batches (<= 65 536 points) first find the table rows they touch and take one of the
+    handle's slots for it: 24 such calls in flight on three streams, each on a different Q^2 band."""
+    torch = torch_cuda
+    pids = [21, 1, -2]
+    rng = np.random.default_rng(99)
+    q_lo, q_hi = np.log(grid2.q2_min), np.log(grid2.q2_max)
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    jobs = []
+    for k in range(24):
+        n = int(rng.integers(1, 6000))
+        a = q_lo + (q_hi - q_lo) * rng.uniform(0, 0.9)
+        b = min(q_hi, a + (q_hi - q_lo) * rng.uniform(0.0, 0.1))
+        x = np.exp(rng.uniform(np.log(grid2.x_knots[0]), 0.0, n))
+        q2 = np.clip(np.exp(rng.uniform(a, b, n)), grid2.q2_min, grid2.q2_max)
+        out = torch.empty((len(pids), n), dtype=torch.float64, device="cuda")
+        jobs.append((x, q2, torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda(), out))
+    for k, (_, _, dx, dq, out) in enumerate(jobs):
+        B.pdf_xfxq2(h2, pids, dx, dq, out, stream=streams[k % 3])
+    torch.cuda.synchronize()
+    for x, q2, _, _, out in jobs:
+        ref, sc = ograph2.xfxq2(pids, x, q2, with_scale=True)
+        check_parity(out.cpu().numpy(), ref, sc, what="row-range slots", log=False)
+
+
+def test_bit_identical_run_to_run(torch_cuda, grid2, h2):
+    """a given batch is bit-reproducible run to run, out-of-grid points included
+    (batch k of a class list is always the warp's entries 32k .. 32k+31, whenever it runs)."""
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    x, q2 = W.queries_extrapolation_mix(grid2, 1_000_003)
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    first = None
+    for _ in range(4):
+        out = torch.full((len(pids), len(x)), float("nan"), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h2, pids, dx, dq, out)
+        torch.cuda.synchronize()
+        if first is None:
+            first = out
+        else:
+            assert torch.equal(out.view(torch.int64), first.view(torch.int64))
+
+
+@pytest.mark.parametrize("pids", [[21], [2, -2, 21, 5, 1]])
+def test_ragged_sizes(torch_cuda, grid2, ograph2, h2, pids):
+    """Sizes around a warp, a tile of 512, one tile per SM, and the small-batch threshold; the tail
+    of every batch holds out-of-grid points (their lists are flushed at the end of the launch).
+    A launch on n points leaves the rest of a longer output buffer alone."""
+    torch = torch_cuda
+    x, q2 = W.queries_extrapolation_mix(grid2, 80_000, config=31)
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    ref, sc = ograph2.xfxq2(pids, x, q2, with_scale=True)
+    for n in (1, 2, 31, 32, 33, 511, 512, 513, 1023, 75_263, 75_264, 75_265, 65_535, 65_536, 65_537, 80_000):
+        dense = torch.empty((len(pids), n), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h2, pids, dx, dq, dense, n=n)
+        torch.cuda.synchronize()
+        got = dense.cpu().numpy()
+        check_parity(got, ref[:, :n], sc[:, :n], max_clause_frac=1.0 if n < 2000 else 5e-3, what=f"ragged n={n}", log=False)
+    # the guard: a launch on n points leaves the rest of a larger buffer alone
+    n = 70_001
+    big = torch.full((len(pids) * n + 4096,), -7.0, dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h2, pids, dx, dq, big, n=n)
+    torch.cuda.synchronize()
+    assert bool((big[len(pids) * n:] == -7.0).all())
