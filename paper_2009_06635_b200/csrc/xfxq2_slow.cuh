@@ -2,7 +2,7 @@
 //
 // The kernel (xfxq2_smem.cu) never evaluates such a point where it occurs.  Each warp appends the
 // point's index to one list per continuation CLASS and evaluates whole batches of 32 entries, one
-// class at a time, when the CTA's flush epoch advances: every call below runs class-uniform on full
+// class at a time, when a list of the CTA reaches the trigger length: every call below runs class-uniform on full
 // warps, and all warps of the CTA run this code at about the same time instead of each alternating
 // with the in-range loop on its own (which thrashed the instruction cache in round 1).
 //

@@ -28,6 +28,8 @@
 
 #include "xfxq2_slow.cuh"
 
+#define PDFB_RR_CACHE_MAX 8192  // SETS: batches up to this size keep their points' (cell, t, tau) in shared memory (24 B each)
+
 template <int MODE, int W>  // compile-time (xfxq2_smem.cuh): a run-time flag costs 11 % (register pressure at the 128 cap)
 __global__ void __launch_bounds__(NT_SMEM, 1)
 k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList pl, long long n,
@@ -101,6 +103,44 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         for (int e = tid; e < npost; e += NT_SMEM) post[e] = __ldg(src + npre + e);
     }
     __syncthreads();
+    // SETS on a small batch (row range known, no point outside the grid): every job of this CTA sees the
+    // SAME points, so the part of a point's evaluation that does not depend on the member table -- both
+    // logarithms, both searches, t and tau -- is done once per CTA and kept in the part of the slice area
+    // that the staged rows leave free: {t, tau} (16 B) and {x interval, Q^2 row} (8 B) per point.  A job
+    // then fetches the two interval records, forms the weights and gathers; results are bit-identical to
+    // the loop below (same lane, same arithmetic).
+    uint32_t cache = 0, cache_i = 0;  // shared addresses of the two arrays; 0 = no cache
+    if constexpr (SETS) {
+        if (row_range && r1 - r0 < g.nq_tot && n <= PDFB_RR_CACHE_MAX) {
+            const int cbytes = (((int)n * 24) + 127) & ~127;
+            const int top = ((shift ? shift + r1 * RBs : lo + stage) + 127) & ~127;
+            int cbase = -1;
+            if (top + cbytes <= slice_bytes) cbase = top;          // above the rows of both buffers
+            else if (cbytes <= lo) cbase = 0;                        // below them
+            if (cbase >= 0) {
+                cache = tab0 + (uint32_t)cbase;
+                cache_i = cache + (uint32_t)(((int)n * 16 + 15) & ~15);
+                const SmemViews sv = make_views<W>(g, smem);
+                const int lane8 = tid & 7;
+                for (int p = tid; p < (int)n; p += NT_SMEM) {
+                    const double xs = __ldg(x + p), qs = load_scale<Q_IS_Q>(q2 + p);
+                    double tx = 0.0, tq = 0.0;
+                    int i = -1, gi = 0;  // i < 0: the point has no value (k_row_range: none is outside the grid)
+                    if (xs >= g.x_min && xs <= g.x_max && qs >= g.q2_min && qs <= g.q2_max) {
+                        const double u = ln_pos(xs), v = ln_pos(qs);
+                        i = locate_x(g, sv, xs, u);
+                        gi = locate_q(g, sv, qs, v);
+                        const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
+                        const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
+                        tx = (u - rx.z0) * rx.inv_dz; tq = (v - rq.z0) * rq.inv_dz;
+                    }
+                    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(cache + (uint32_t)p * 16u), "d"(tx), "d"(tq) : "memory");
+                    asm volatile("st.shared.v2.s32 [%0], {%1, %2};" ::"r"(cache_i + (uint32_t)p * 8u), "r"(i), "r"(gi) : "memory");
+                }
+                __syncthreads();
+            }
+        }
+    }
     int jj = 0;
     do {  // jobs of this CTA (one, unless SETS)
     const int buf = shift ? (jj & 1) : 0;
@@ -129,9 +169,9 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     // every call is class-uniform on full lanes; a remainder stays at the front of its list, so batch
     // k of a class is always the warp's entries 32k .. 32k+31 of that class, whenever it is evaluated
     // (results do not depend on timing).  WHEN: a warp whose list reaches PDFB_SLOW_TRIGGER entries
-    // advances the CTA's flush epoch; every warp compares the epoch once per tile and evaluates its
-    // full batches when it has moved -- all warps run the out-of-grid code at about the same time,
-    // without a barrier (a barrier every few tiles costs the in-range loop 7-25 %, measured).
+    // raises a request flag for every warp of the CTA; a warp that holds entries looks at its flag once
+    // per tile and then evaluates its full batches -- all warps run the out-of-grid code at about the
+    // same time, without a barrier (a barrier every few tiles costs the in-range loop 7-25 %, measured).
     // The lists live in a global scratch slot owned by this SM: at most one CTA of this kernel is
     // resident per SM, on any stream, because the launcher requests more than half of the SM's shared
     // memory (checked at load: occupancy == 1).
@@ -145,6 +185,27 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
         flush_warp_lists<MODE, W>(final, wlist(), &wcnt[threadIdx.x >> 5][0], &s_req[threadIdx.x >> 5], &g, smem, x, q2, out, out_stride, n_req, pl.row[pass]);
     };
 
+    if (SETS && cache) {  // the points' table-independent part comes from the cache (above)
+        for (int p = tid; p < (int)n; p += NT_SMEM) {
+            const double2 tt = lds128(cache + (uint32_t)p * 16u);
+            int i, gi;
+            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(i), "=r"(gi) : "r"(cache_i + (uint32_t)p * 8u));
+            double y[W];
+            if (i >= 0) {
+                const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);
+                const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
+                double wu[4], vw[4];
+                weights_rec32(rx, tt.x, wu);
+                weights_rec32(rq, tt.y, vw);
+                eval_stencil<W>(tab, RB, rb2, rb3, gi - 1, i - 1, wu, vw, lane8, y);
+            } else {
+#pragma unroll
+                for (int c = 0; c < W; c++) y[c] = qnan;
+                if (job == 0) atomicAdd(g.n_invalid, 1ULL);
+            }
+            store_cols<W, OUT>(out, out_stride, n_req, p, row, y);
+        }
+    } else {
     bool pending = false;  // this warp has list entries (the flush request is only looked at then)
     // software pipeline: the next tile's coordinates are in flight while this tile is evaluated
     long long tile = seq;
@@ -234,6 +295,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     if (pending) { flush_lists(false); pending = false; }
     }
     flush_lists(true);
+    }
     if (SETS) {
         __syncthreads();  // every warp is done with this job's rows (measured: mbarrier hand-over between the warps
                           // instead of this barrier changes nothing -- a job is bound by its five tile iterations)
@@ -246,11 +308,9 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 // Rows of the concatenated Q^2 knot list that a batch can touch: the intervals of its smallest and
 // largest in-range Q^2, two rows below and three above (the 4-row stencils and their zero-weight
 // overreach); the whole table as soon as one point lies outside the grid (the out-of-grid classes read
-// fixed rows at either end and locate the table themselves).  (old text follows)
-// 
-// one Q^2 lies outside the grid (rules B and C read fixed rows at either end).  One CTA; for batches
-// small enough that staging the whole 200 KB slice per CTA costs as much as evaluating them
-// (PDF sets on an x-grid at one scale: 2415 points, 4 rows of 64).
+// fixed rows at either end and locate the table themselves).  One CTA; for batches small enough that
+// staging the whole 200 KB slice per CTA costs as much as evaluating them (PDF sets on an x-grid at
+// one scale: 2415 points, 6 rows of 64).
 template <bool Q_IS_Q>
 __global__ void __launch_bounds__(1024) k_row_range(const GridDev g, long long n, const double *__restrict__ x,
                                                     const double *__restrict__ q2, int *__restrict__ rr)

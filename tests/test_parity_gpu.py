@@ -297,6 +297,28 @@ def test_member_set(torch_cuda):
     torch.cuda.synchronize()
     ref, sc = oracle.xfxq2_members(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals, pids, x, q2, with_scale=True)
     check_parity(out.cpu().numpy(), ref, sc, what="member set, FK x-grid")
+    # the set kernel keeps the points' (cell, t, tau) in shared memory across its jobs; a member loaded
+    # on its own goes through the ordinary loop: same lanes, same arithmetic, so bit for bit the same
+    for m in (0, 5, n_mem - 1):
+        h1 = B.pdf_grid_load(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals[m])
+        o1 = torch.empty((len(pids), len(x)), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h1, pids, dx, dq, o1)
+        torch.cuda.synchronize()
+        assert torch.equal(o1.view(torch.int64), out[m].view(torch.int64)), m
+        B.pdf_grid_free(h1)
+    # a batch with invalid points (no value: NaN, counted once per point) still takes the cached path
+    xb, qb = x.copy(), q2.copy()
+    xb[[3, 700, 2414]] = [np.nan, 1.5, -1.0]
+    qb[[9, 1000]] = [0.0, np.inf]
+    ob = torch.empty((n_mem, len(pids), len(x)), dtype=torch.float64, device="cuda")
+    before = B.pdf_grid_status(h)
+    B.pdf_xfxq2_members(h, 0, n_mem, pids, torch.from_numpy(xb).cuda(), torch.from_numpy(qb).cuda(), ob)
+    torch.cuda.synchronize()
+    assert B.pdf_grid_status(h) - before == 5
+    bad = np.zeros(len(x), dtype=bool)
+    bad[[3, 700, 2414, 9, 1000]] = True
+    got = ob.cpu().numpy()
+    assert np.isnan(got[:, :, bad]).all() and np.array_equal(got[:, :, ~bad], out.cpu().numpy()[:, :, ~bad])
     # a member range in the middle, a PID subset, the extrapolation mix (few jobs: persistent CTAs)
     xm, qm = W.queries_extrapolation_mix(g0, 20_011)
     sub = [21, -6, 2]
