@@ -203,6 +203,29 @@ def timed_reps(torch, fn, reps=20, warm=3):
     return {"ms": float(np.median(ts)), "ms_best": ts[0], "reps": reps}
 
 
+def graph_replay_ms(torch, fn, per_graph=20, reps=10):
+    """Device time of one fn() when `per_graph` of them are captured into ONE CUDA graph and replayed:
+    what a launch-latency-sized call costs inside a captured loop (the calls allocate nothing and never
+    synchronise, so they can be captured).  Median over `reps` replays, per call."""
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        fn()
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        for _ in range(per_graph):
+            fn()
+    g.replay()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for a, b in ev:
+        a.record(); g.replay(); b.record()
+    torch.cuda.synchronize()
+    return float(np.median([a.elapsed_time(b) for a, b in ev])) / per_graph
+
+
 def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s):
     """Configs 1, 2, 4 and 5 of BASELINE.json at their full sizes, device-resident, reported beside
     the metric (parity-test cases, not the headline): median and best of 20 CUDA-event timings, each
@@ -222,12 +245,14 @@ def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s):
     h1 = B.load_pdf_spec(g1)
     x, q2 = dev(*W.queries_in_range(g1, 10_000, 1))
     o = torch.empty((3, 10_000), dtype=torch.float64, device="cuda")
-    res["config1_1e4x3"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2(h1, list(W.PIDS_3), x, q2, o)), 10_000, 3, 40, w_in(3),
-                                 note="launch-latency sized")
+    f1 = lambda: B.pdf_xfxq2(h1, list(W.PIDS_3), x, q2, o)
+    res["config1_1e4x3"] = entry(timed_reps(torch, f1), 10_000, 3, 40, w_in(3), note="launch-latency sized",
+                                 ms_in_cuda_graph=graph_replay_ms(torch, f1))
     B.pdf_grid_free(h1)
     x, q2 = dev(*W.queries_in_range(grid, 1_000_000, 2))
     o = torch.empty((11, 1_000_000), dtype=torch.float64, device="cuda")
-    res["config2_1e6x11"] = entry(timed_reps(torch, lambda: B.pdf_xfxq2(h, p11, x, q2, o)), 1_000_000, 11, 104, w_in(11))
+    f2 = lambda: B.pdf_xfxq2(h, p11, x, q2, o)
+    res["config2_1e6x11"] = entry(timed_reps(torch, f2), 1_000_000, 11, 104, w_in(11), ms_in_cuda_graph=graph_replay_ms(torch, f2))
     n4 = 10_000_000
     x, q2 = dev(*W.queries_extrapolation_mix(grid, n4))
     o = torch.empty((11, n4), dtype=torch.float64, device="cuda")

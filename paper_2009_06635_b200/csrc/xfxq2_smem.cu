@@ -134,6 +134,7 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
                         const IntervalRec32 rq = load_rec4(sv.qrec + (uint32_t)gi * 128u, lane8);
                         tx = (u - rx.z0) * rx.inv_dz; tq = (v - rq.z0) * rq.inv_dz;
                     }
+                    PDFB_ASSERT(cache_i + (uint32_t)p * 8u + 8u <= tab0 + (uint32_t)slice_bytes);
                     asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(cache + (uint32_t)p * 16u), "d"(tx), "d"(tq) : "memory");
                     asm volatile("st.shared.v2.s32 [%0], {%1, %2};" ::"r"(cache_i + (uint32_t)p * 8u), "r"(i), "r"(gi) : "memory");
                 }
@@ -188,8 +189,8 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     if (SETS && cache) {  // the points' table-independent part comes from the cache (above)
         for (int p = tid; p < (int)n; p += NT_SMEM) {
             const double2 tt = lds128(cache + (uint32_t)p * 16u);
-            int i, gi;
-            asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(i), "=r"(gi) : "r"(cache_i + (uint32_t)p * 8u));
+            const int2 cell = lds64i(cache_i + (uint32_t)p * 8u);
+            const int i = cell.x, gi = cell.y;
             double y[W];
             if (i >= 0) {
                 const IntervalRec32 rx = load_rec4(sv.xrec + (uint32_t)i * 128u, lane8);

@@ -46,6 +46,16 @@ __device__ __forceinline__ double2 lds128(uint32_t addr)
     return v;
 }
 
+__device__ __forceinline__ int2 lds64i(uint32_t addr)
+{
+#ifdef PDFB_CHECKED
+    pdfb_check_smem(addr, 8);
+#endif
+    int2 v;
+    asm volatile("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+
 // The four 1-D weights of knots m-1..m+2 from the 32-byte interval record.  aLm == 0 marks the
 // first interval of the knot array (knot m-1 does not exist, weight exactly 0), aHp == 0 the last.
 __device__ __forceinline__ void weights_rec32(const IntervalRec32 &r, double t, double w[4])

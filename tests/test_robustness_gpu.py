@@ -125,3 +125,58 @@ def test_ragged_sizes(torch_cuda, grid2, ograph2, h2, pids):
     B.pdf_xfxq2(h2, pids, dx, dq, big, n=n)
     torch.cuda.synchronize()
     assert bool((big[len(pids) * n:] == -7.0).all())
+
+
+def test_calls_can_be_captured_in_a_cuda_graph(torch_cuda, grid2, ograph2, h2):
+    """include/pdfb200.h: the evaluation calls allocate nothing and never synchronise.  A launch-bound
+    loop can therefore be captured once and replayed: pdf_xfxq2 (a small batch, which also runs the
+    row-range pre-pass), pdf_xfxq2 on an extrapolation mix, alphas_q2 and pdf_lumi_events in ONE graph;
+    after the inputs are overwritten in place, a replay gives bit for bit what direct calls give."""
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    aspec = W.make_alphas_grid()
+    ha = B.load_alphas_spec(aspec)
+    n_s, n_m = 3_001, 150_001
+    terms = [(1, -1, 1.0), (-2, 2, 0.5), (21, 21, 0.25)]
+
+    def inputs(k):
+        xs, qs = W.queries_in_range(grid2, n_s, 40 + k)
+        xm, qm = W.queries_extrapolation_mix(grid2, n_m, config=50 + k)
+        x1, x2, qe = W.queries_mc_events(grid2, n_m, config=60 + k)
+        return [torch.from_numpy(a).cuda() for a in (xs, qs, xm, qm, x1, x2, qe)]
+
+    buf = inputs(0)
+    xs, qs, xm, qm, x1, x2, qe = buf
+    o_s = torch.empty((len(pids), n_s), dtype=torch.float64, device="cuda")
+    o_m = torch.empty((len(pids), n_m), dtype=torch.float64, device="cuda")
+    o_a = torch.empty(n_m, dtype=torch.float64, device="cuda")
+    o_l = torch.empty(n_m, dtype=torch.float64, device="cuda")
+
+    def calls(os_, om_, oa_, ol_):
+        B.pdf_xfxq2(h2, pids, xs, qs, os_)
+        B.pdf_xfxq2(h2, pids, xm, qm, om_)
+        B.alphas_q2(ha, qe, oa_)
+        B.pdf_lumi_events(h2, terms, x1, x2, qe, ol_)
+
+    calls(o_s, o_m, o_a, o_l)  # first use outside the capture (function attributes are set on first use)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        calls(o_s, o_m, o_a, o_l)
+    for k in (1, 2):
+        for dst, src in zip(buf, inputs(k)):
+            dst.copy_(src)
+        for o in (o_s, o_m, o_a, o_l):
+            o.fill_(float("nan"))
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        d = [torch.empty_like(o) for o in (o_s, o_m, o_a, o_l)]
+        calls(*d)
+        torch.cuda.synchronize()
+        for got, want in zip((o_s, o_m, o_a, o_l), d):
+            assert torch.equal(got.view(torch.int64), want.view(torch.int64)), k
+    ref, sc = ograph2.xfxq2(pids, xs.cpu().numpy(), qs.cpu().numpy(), with_scale=True)
+    check_parity(o_s.cpu().numpy(), ref, sc, what="graph replay, small batch")
+    B.alphas_grid_free(ha)
