@@ -180,3 +180,38 @@ def test_calls_can_be_captured_in_a_cuda_graph(torch_cuda, grid2, ograph2, h2):
     ref, sc = ograph2.xfxq2(pids, xs.cpu().numpy(), qs.cpu().numpy(), with_scale=True)
     check_parity(o_s.cpu().numpy(), ref, sc, what="graph replay, small batch")
     B.alphas_grid_free(ha)
+
+
+def test_more_than_2_to_the_31_points(torch_cuda, grid2, ograph2, h2):
+    """Maximum sizes: the class lists hold point indices as 32-bit offsets, so a batch beyond 2^31 points
+    goes out in slices of 2^31 (xfxq2_smem.cu).  2^31 + 70 001 points, PID 21, a fifth of them below
+    x_min: sampled against the oracle at both ends, across the slice boundary and at random."""
+    torch = torch_cuda
+    n = (1 << 31) + 70_001
+    free, _ = torch.cuda.mem_get_info()
+    if free < 3 * 8 * n + (8 << 30):
+        pytest.skip("needs ~60 GB of free device memory")
+    gen = torch.Generator(device="cuda").manual_seed(2009_06635)
+    x = torch.empty(n, dtype=torch.float64, device="cuda")
+    q2 = torch.empty(n, dtype=torch.float64, device="cuda")
+    lx0, lq0, lq1 = np.log(float(grid2.x_knots[0])), np.log(grid2.q2_min), np.log(grid2.q2_max)
+    step = 1 << 27
+    for a in range(0, n, step):  # ln x uniform on [ln x_min - 5, 0]: about a fifth of the points below x_min
+        b = min(n, a + step)
+        x[a:b].uniform_(lx0 - 5.0, 0.0, generator=gen).exp_()
+        q2[a:b].uniform_(lq0, lq1, generator=gen).exp_().clamp_(grid2.q2_min, grid2.q2_max)
+    out = torch.full((1, n), -7.0, dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h2, [21], x, q2, out)
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(5)
+    idx = np.unique(np.concatenate([np.arange(0, 2000), np.arange((1 << 31) - 3000, (1 << 31) + 3000), np.arange(n - 2000, n),
+                                    rng.integers(0, n, 40_000)]))
+    sel = torch.from_numpy(idx).cuda()
+    xs, qs, got = x[sel].cpu().numpy(), q2[sel].cpu().numpy(), out[0, sel].cpu().numpy()
+    ref, sc = ograph2.xfxq2([21], xs, qs, with_scale=True)
+    st = check_parity(got[None, :], ref, sc, max_clause_frac=5e-3, what="2^31 + 70001 points")
+    print("2^31 points", st, "below x_min in the sample:", float((xs < grid2.x_knots[0]).mean()))
+    assert float((xs < grid2.x_knots[0]).mean()) > 0.1
+    # nothing was left unwritten: no -7 anywhere (chunked, the array is 17 GB)
+    for a in range(0, n, step):
+        assert not bool((out[0, a:min(n, a + step)] == -7.0).any())
