@@ -719,3 +719,43 @@ def test_per_subgrid_x_knots_are_independent_grids():
                                x_offsets=np.arange(4, dtype=np.int32) * len(xk))
     x = np.exp(rng.uniform(np.log(1e-7), 0.0, 2000)); q2 = np.exp(rng.uniform(np.log(0.5), np.log(2e6), 2000))
     assert np.array_equal(shared.xfxq2(pids, x, q2), per.xfxq2(pids, x, q2), equal_nan=True)
+
+
+def test_C1_inside_a_subgrid_and_a_kink_only_at_thresholds():
+    """A cubic Hermite interpolant with ONE derivative per knot (reading O2) is C1: along either axis the
+    slope just left of an interior knot equals the slope just right of it, on random non-uniform knots
+    and random values.  Across a Q^2 threshold the sub-grids are interpolated independently (P2), so
+    there -- and only there -- the slope may jump.  (A derivative rule that differs between the two
+    cells sharing a knot, or a stencil shifted by one, shows up as a kink of order 1.)"""
+    rng = np.random.default_rng(42)
+    xk = rand_knots(rng, 1e-5, 1.0, 9)
+    subs = [rand_knots(rng, 1.5, 4.0, 5), rand_knots(rng, 4.0, 90.0, 7)]
+    vals = [rng.normal(size=(len(xk), len(q), 1)) for q in subs]
+    vals[1][:, 0, :] = vals[0][:, -1, :]   # the same values on both copies of the threshold knot: f itself is continuous there
+    g = oracle.OraclePdfGrid.from_spec(make_spec(xk, subs, [21], values=vals))
+    e = 1e-6
+
+    def slopes_x(xknot, q2):   # d f / d ln x just left and just right of the knot
+        pts = np.array([xknot * np.exp(-e), xknot, xknot * np.exp(e)])
+        f = g.xfxq2([21], pts, np.full(3, q2))[0]
+        return (f[1] - f[0]) / e, (f[2] - f[1]) / e
+
+    def slopes_q(x, q2knot):
+        pts = np.array([q2knot * np.exp(-e), q2knot, q2knot * np.exp(e)])
+        f = g.xfxq2([21], np.full(3, x), pts)[0]
+        return (f[1] - f[0]) / e, (f[2] - f[1]) / e
+
+    for q in (subs[0][1] ** 2 * 1.3, subs[1][3] ** 2 * 1.1):
+        for xn in xk[1:-1]:
+            l, r = slopes_x(xn, q)
+            assert abs(l - r) < 2e-4 * max(1.0, abs(l)), (xn, l, r)
+    jumps = []
+    for x in (xk[2] * 1.2, xk[6] * 1.05):
+        for s, qs in enumerate(subs):
+            for qn in qs[1:-1]:
+                l, r = slopes_q(x, qn ** 2)
+                assert abs(l - r) < 2e-4 * max(1.0, abs(l)), (x, qn, l, r)
+        l, r = slopes_q(x, subs[1][0] ** 2)   # the threshold: last knot of sub-grid 0 = first of sub-grid 1
+        assert abs(l) < 1e3 and abs(r) < 1e3   # no jump of the value (that would be a slope ~ 1/e)
+        jumps.append(abs(l - r))
+    assert max(jumps) > 1e-2  # random values: the one-sided slopes of two independent sub-grids differ
