@@ -52,13 +52,19 @@ k_alphas(AlphasDev A, long long n, const double *__restrict__ q2, double *__rest
 }
 
 // Fast path (K <= 192 nodes): replicated coefficient lines in shared memory, LUT location,
-// one cubic in s = ln Q^2 - Z_m per point (five doubles per interval: two LDS.128 and one LDS.64), ln Q^2 through a 64-entry table (ln_tab, pdfb_internal.cuh).  Four points per
-// thread and iteration; 3 CTAs of 512 threads per SM (48 KB of tables each).
+// one cubic in s = ln Q^2 - Z_m per point (five doubles per interval: two LDS.128 and one LDS.64),
+// ln Q^2 through a 64-entry table (ln_tab, pdfb_internal.cuh).  Six points per thread and iteration;
+// 2 CTAs of 768 threads per SM (48 KB of tables each).  Measured per 1e8 points (threads x CTAs x
+// points): 512 x 3 x 4: 0.328 ms, 512 x 3 x 8: 0.324, 768 x 2 x 4: 0.320, 768 x 2 x 6: 0.312 (kept),
+// 768 x 2 x 8: 0.312, 640 x 2 x 6: 0.324, 1024 x 1 x 8: 0.333, 384 x 4 x 4: 0.332, 256 x 6 x 4: 0.436.
 #ifndef NT_ALPHAS
-#define NT_ALPHAS 512
+#define NT_ALPHAS 768
 #endif
 #ifndef CTAS_ALPHAS
-#define CTAS_ALPHAS 3
+#define CTAS_ALPHAS 2
+#endif
+#ifndef PTS_ALPHAS
+#define PTS_ALPHAS 6   // points per thread and iteration
 #endif
 
 template <bool Q_IS_Q>
@@ -103,19 +109,19 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
         }
         return (qv > 0.0) ? res : qnan;  // NaN and non-positive Q^2 have no value
     };
-    // 4 points per thread and iteration: the loads go out together, the ln chains interleave.
+    // PTS_ALPHAS points per thread and iteration: the loads go out together, the ln chains interleave.
     // (Measured and dropped: the four points evaluated stage by stage without branches between the
     // stages -- all table loads of a stage issued together -- 0.345 ms against 0.330 ms per 1e8 points.)
     const long long stride = (long long)gridDim.x * NT_ALPHAS;
     long long p = blockIdx.x * (long long)NT_ALPHAS + threadIdx.x;
-    for (; p + 3 * stride < n; p += 4 * stride) {
-        double q[4], r[4];
+    for (; p + (PTS_ALPHAS - 1) * stride < n; p += PTS_ALPHAS * stride) {
+        double q[PTS_ALPHAS], r[PTS_ALPHAS];
 #pragma unroll
-        for (int k = 0; k < 4; k++) q[k] = __ldcs(q2 + p + k * stride);
+        for (int k = 0; k < PTS_ALPHAS; k++) q[k] = __ldcs(q2 + p + k * stride);
 #pragma unroll
-        for (int k = 0; k < 4; k++) r[k] = eval(q[k]);
+        for (int k = 0; k < PTS_ALPHAS; k++) r[k] = eval(q[k]);
 #pragma unroll
-        for (int k = 0; k < 4; k++) __stcs(out + p + k * stride, r[k]);
+        for (int k = 0; k < PTS_ALPHAS; k++) __stcs(out + p + k * stride, r[k]);
     }
     for (; p < n; p += stride) __stcs(out + p, eval(__ldcs(q2 + p)));
 }
