@@ -226,7 +226,7 @@ def graph_replay_ms(torch, fn, per_graph=20, reps=10):
     return float(np.median([a.elapsed_time(b) for a, b in ev])) / per_graph
 
 
-def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s):
+def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s, graph=True):
     """Configs 1, 2, 4 and 5 of BASELINE.json at their full sizes, device-resident, reported beside
     the metric (parity-test cases, not the headline): median and best of 20 CUDA-event timings, each
     with its fraction of the slower contract bound."""
@@ -246,13 +246,13 @@ def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s):
     x, q2 = dev(*W.queries_in_range(g1, 10_000, 1))
     o = torch.empty((3, 10_000), dtype=torch.float64, device="cuda")
     f1 = lambda: B.pdf_xfxq2(h1, list(W.PIDS_3), x, q2, o)
-    res["config1_1e4x3"] = entry(timed_reps(torch, f1), 10_000, 3, 40, w_in(3), note="launch-latency sized",
-                                 ms_in_cuda_graph=graph_replay_ms(torch, f1))
+    gr = (lambda f: {"ms_in_cuda_graph": graph_replay_ms(torch, f)}) if graph else (lambda f: {})
+    res["config1_1e4x3"] = entry(timed_reps(torch, f1), 10_000, 3, 40, w_in(3), note="launch-latency sized", **gr(f1))
     B.pdf_grid_free(h1)
     x, q2 = dev(*W.queries_in_range(grid, 1_000_000, 2))
     o = torch.empty((11, 1_000_000), dtype=torch.float64, device="cuda")
     f2 = lambda: B.pdf_xfxq2(h, p11, x, q2, o)
-    res["config2_1e6x11"] = entry(timed_reps(torch, f2), 1_000_000, 11, 104, w_in(11), ms_in_cuda_graph=graph_replay_ms(torch, f2))
+    res["config2_1e6x11"] = entry(timed_reps(torch, f2), 1_000_000, 11, 104, w_in(11), **gr(f2))
     n4 = 10_000_000
     x, q2 = dev(*W.queries_extrapolation_mix(grid, n4))
     o = torch.empty((11, n4), dtype=torch.float64, device="cuda")
@@ -457,7 +457,7 @@ def run_gpu(args):
             "alphas": {"points": n, "ms": a_t["ms"], "ms_best": a_t["ms_best"], "evaluations_per_s": n / (a_t["ms"] * 1e-3),
                        **roofline_entry(a_t["ms"], n, 16, 48, peak, fma_ps)}}
     if not args.no_other_configs:
-        line["other_configs"] = bench_other_configs(torch, B, h, ha, grid, peak, fma_ps)
+        line["other_configs"] = bench_other_configs(torch, B, h, ha, grid, peak, fma_ps, graph=not args.no_graph)
     B.alphas_grid_free(ha)
     if not args.no_members:
         line["multi_member"] = bench_members(torch, B, local, args.members)
@@ -536,6 +536,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-members", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="skip the CUDA-graph replay timings of configs 1 and 2 (the ncu launch list)")
     ap.add_argument("--no-other-configs", action="store_true")
     ap.add_argument("--members", type=int, default=400, help="N_rep of the multi-member leg (Table 2)")
     ap.add_argument("--leg", default=None, help="profiling aid: run only config4 | config4_f1 | lumi | alphas | members")
