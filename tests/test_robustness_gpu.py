@@ -215,3 +215,44 @@ def test_more_than_2_to_the_31_points(torch_cuda, grid2, ograph2, h2):
     # nothing was left unwritten: no -7 anywhere (chunked, the array is 17 GB)
     for a in range(0, n, step):
         assert not bool((out[0, a:min(n, a + step)] == -7.0).any())
+
+
+def test_host_threads_share_one_handle(torch_cuda, grid2, h2):
+    """Four host threads (ctypes releases the GIL during a call), each on its own stream, launch small
+    and large batches on ONE handle at the same time: the handle's only mutable host state is the
+    round-robin slot counter (atomic) and the per-function attribute flags (atomic).  Every result
+    equals the one the same call gives on its own."""
+    import threading
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    work = []
+    for k, n in enumerate((2_001, 40_003, 300_007, 5)):
+        x, q2 = W.queries_extrapolation_mix(grid2, n, config=8000 + k)
+        dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+        want = torch.empty((len(pids), n), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h2, pids, dx, dq, want)
+        work.append((dx, dq, want))
+    torch.cuda.synchronize()
+    errors = []
+
+    def run(k):
+        try:
+            dx, dq, want = work[k]
+            s = torch.cuda.Stream()
+            for _ in range(40):
+                out = torch.full_like(want, float("nan"))
+                s.wait_stream(torch.cuda.current_stream())
+                B.pdf_xfxq2(h2, pids, dx, dq, out, stream=s)
+                s.synchronize()
+                if not torch.equal(out.view(torch.int64), want.view(torch.int64)):
+                    errors.append(k)
+                    return
+        except Exception as e:  # noqa: BLE001 -- reported below, from the main thread
+            errors.append((k, repr(e)))
+
+    threads = [threading.Thread(target=run, args=(k,)) for k in range(len(work))]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
