@@ -276,18 +276,6 @@ int pdfb_lhapdf_info_alphas(const char *info_path, int cap, double *q_knots, dou
 /* NumMembers of a set's metadata file (1 if the key is absent). */
 int pdfb_lhapdf_info_members(const char *info_path, int *n_members);
 
-/*
- * pdfb_probe -- machine probes for the bounds MEASURED_PEAKS.json does not carry (SURVEY.md 8(d):
- * the FP64 peak must be measured).  Not part of the method; used by bench.py only.
- *   PDFB_PROBE_FP64  *result = FP64 fused multiply-adds per second (thread level) of independent
- *                    DFMA chains at full occupancy
- *   PDFB_PROBE_LDS   *result = bytes per second delivered by conflict-free LDS.128 from shared memory
- * Synchronous; allocates and frees its own scratch.  result: host pointer.
- */
-#define PDFB_PROBE_FP64 1
-#define PDFB_PROBE_LDS 2
-int pdfb_probe(int which, int device, double *result);
-
 #ifdef __cplusplus
 }
 #endif

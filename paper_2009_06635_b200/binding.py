@@ -22,7 +22,7 @@ _ll = ctypes.c_longlong
 
 EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
-           "pdfb_launch_count", "pdfb_probe", "pdf_lumi_events", "pdf_xfxq2_pm", "pdf_xfxq2_f32", "pdf_grid_load_xs", "pdfb_lhagrid_dims_xs", "pdfb_lhagrid_get_xs", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
+           "pdfb_launch_count", "pdf_lumi_events", "pdf_xfxq2_pm", "pdf_xfxq2_f32", "pdf_grid_load_xs", "pdfb_lhagrid_dims_xs", "pdfb_lhagrid_get_xs", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
            "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
 
 
@@ -99,8 +99,6 @@ def lib():
         L.pdfb_lhapdf_info_alphas.argtypes = [ctypes.c_char_p, ctypes.c_int, _dp, _dp, _ip]
         L.pdfb_lhapdf_info_members.restype = ctypes.c_int
         L.pdfb_lhapdf_info_members.argtypes = [ctypes.c_char_p, _ip]
-        L.pdfb_probe.restype = ctypes.c_int
-        L.pdfb_probe.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
         L.pdfb_debug_ln.restype = ctypes.c_int
         L.pdfb_debug_ln.argtypes = [_vp, _vp, _ll, _vp]
         _lib = L
@@ -118,11 +116,23 @@ def launch_count() -> int:
 PROBE_FP64, PROBE_LDS = 1, 2
 
 
+_probe_lib = None
+
+
 def probe(which: int, device: int = 0) -> float:
-    """Machine probe (pdfb200.h): FP64 FMA/s or shared-memory bytes/s."""
+    """Machine probe (include/pdfb200_probe.h, libpdfb200_probe.so -- a bench utility, not part of the
+    product library): FP64 FMA/s or shared-memory bytes/s."""
+    global _probe_lib
+    if _probe_lib is None:
+        path = os.path.join(_HERE, "libpdfb200_probe.so")
+        if not os.path.exists(path):
+            raise RuntimeError(f"{path} is missing: build it with `python -m paper_2009_06635_b200.build`")
+        _probe_lib = ctypes.CDLL(path)
+        _probe_lib.pdfb_probe.restype = ctypes.c_int
+        _probe_lib.pdfb_probe.argtypes = [ctypes.c_int, ctypes.c_int, _dp]
     r = ctypes.c_double(0.0)
-    _check(lib().pdfb_probe(int(which), int(device), ctypes.byref(r)), "pdfb_probe")
-    return float(r.value)
+    _check(_probe_lib.pdfb_probe(int(which), int(device), ctypes.byref(r)), "pdfb_probe")
+    return r.value
 
 
 def debug_ln(x, out, stream=None):

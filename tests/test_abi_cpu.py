@@ -26,6 +26,19 @@ def test_exports_every_declared_symbol(L):
     for n in names:
         assert hasattr(L, n), n
     assert set(B.EXPORTS) <= names
+    assert "pdfb_probe" not in names and not hasattr(L, "pdfb_probe")  # the bench's machine probes are not in the product library
+
+
+def test_probe_library_exports_its_header(L):
+    """include/pdfb200_probe.h is served by libpdfb200_probe.so, a library of its own."""
+    import ctypes
+    hdr = open(os.path.join(ROOT, "include", "pdfb200_probe.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(pdfb_\w+)\s*\(", hdr))
+    assert names == {"pdfb_probe"}
+    P = ctypes.CDLL(build.PROBE_LIB)
+    for n in names:
+        assert hasattr(P, n), n
 
 
 def test_strerror_and_codes(L):
