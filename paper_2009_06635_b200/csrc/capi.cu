@@ -142,8 +142,9 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     d.a_xrec = (int)align_up(d.a_q2k + sizeof(double) * nq_tot, 128);
     d.pre_bytes = d.a_xrec + 128 * nx;            // the slice starts here, 128-byte aligned
     d.a_qrec = 0;
-    // a stencil may reach one row plus three knots past the table: keep that much finite data there
-    d.post_bytes = (int)align_up((size_t)std::max(128 * nq_tot, d.nx4 * 32 + 128), 128);
+    // a stencil may reach two rows plus three knots past the table (the phantom interval of the last Q^2
+    // knot, xfxq2_smem.cuh): keep that much finite data there
+    d.post_bytes = (int)align_up((size_t)std::max(128 * nq_tot, 2 * d.nx4 * 32 + 128), 128);
     if (128 * nx < d.nx4 * 32 + 32) d.smem_ok = 0;  // (never: 128 nx >= 32 nx4 + 32 for nx >= 2)
     const int aux_bytes = d.pre_bytes + d.post_bytes;
     // which layouts this handle will ever read (a set of 400 members is ~1 GB if all are kept):
@@ -197,8 +198,8 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
             const double *U = h_z.data(), *V = h_z.data() + nx;
             d.lutx_u0 = U[0]; d.lutx_inv_h = PDFB_LUT_BINS / (U[nx - 1] - U[0]);
             d.lutq_v0 = V[0]; d.lutq_inv_h = PDFB_LUT_BINS / (V[nq_tot - 1] - V[0]);
-            pdfb_fill_lut(lx, U, x_knots, nx, nx - 2);          // the last x knot starts no interval
-            pdfb_fill_lut(lq, V, h_q2.data(), nq_tot, nq_tot - 1);  // concatenated Q^2 knots; clamped after the search
+            pdfb_fill_lut(lx, U, x_knots, nx, nx - 1);          // (the last knot starts its phantom interval, xfxq2_smem.cuh)
+            pdfb_fill_lut(lq, V, h_q2.data(), nq_tot, nq_tot - 1);  // concatenated Q^2 knots
             if (cudaMemcpy(blob + o_aux, aux.data(), aux_bytes, cudaMemcpyHostToDevice) != cudaSuccess) { rc = PDFB_ECUDA; break; }
         }
         rc = pdfb_setup_records((const double *)(blob + o_z), (IntervalRec *)(blob + o_xrec),

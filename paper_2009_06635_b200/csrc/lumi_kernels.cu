@@ -102,7 +102,7 @@ k_lumi_band(const __grid_constant__ GridDev g, const __grid_constant__ LumiCoef 
         for (int e = tid; e < npre; e += LUMI_NT) pre[e] = __ldg(src + e);
         for (int e = tid; e < nqr; e += LUMI_NT) qr[e] = __ldg(src + npre + e);
         int4 *bz = reinterpret_cast<int4 *>(smem + L.l_band);
-        for (int e = tid; e < NPAIR * L.pair_stride / 16; e += LUMI_NT) bz[e] = make_int4(0, 0, 0, 0);
+        for (int e = tid; e < (L.l_qrec - L.l_band) / 16; e += LUMI_NT) bz[e] = make_int4(0, 0, 0, 0);  // the pairs' areas and the tail pad
 #ifdef PDFB_CHECKED
         // poison what a band will overwrite (the rows of the pairs that exist): only a pair that does not exist
         // and the alignment row keep their zeros
@@ -286,7 +286,10 @@ int pdfb_lumi_plan(pdfb_grid *g)
     L.ncell = d.nq_tot - 1;
     const int qrec_bytes = 128 * d.nq_tot;
     const int list_bytes = (LUMI_NT / 32) * LUMI_LIST * (3 * 8 + 4);
-    const int avail = dev_max - LUMI_STATIC_SMEM - d.pre_bytes - qrec_bytes - list_bytes - 256;
+    // the stencil of the last knot's phantom interval (xfxq2_smem.cuh) reaches two rows and three knots past a pair's
+    // rows with weight 0: the next pair's rows for all pairs but the last, a pad of zeros after the last
+    const int tail_pad = (2 * L.RB2 + 3 * 16 + 127) & ~127;
+    const int avail = dev_max - LUMI_STATIC_SMEM - d.pre_bytes - qrec_bytes - list_bytes - tail_pad - 256;
     int R = avail / (npair * L.RB2);
     R &= ~1;                                   // even: the pair stride stays a multiple of 128 bytes
     if (R >= d.nq_tot) { L.R = d.nq_tot; L.R_alloc = (d.nq_tot + 1) & ~1; L.CB = L.ncell; }
@@ -295,7 +298,7 @@ int pdfb_lumi_plan(pdfb_grid *g)
     L.n_bands = (L.ncell + L.CB - 1) / L.CB;
     L.pair_stride = L.R_alloc * L.RB2;
     L.l_band = d.pre_bytes;                    // 128-byte aligned (pre ends with the 128-byte xrec lines)
-    L.l_qrec = L.l_band + npair * L.pair_stride;
+    L.l_qrec = L.l_band + npair * L.pair_stride + tail_pad;
     L.l_list = L.l_qrec + qrec_bytes;
     L.total = L.l_list + list_bytes;
     if (L.total + LUMI_STATIC_SMEM > dev_max || (L.pair_stride & 127) || (L.l_band & 127)) return PDFB_OK;

@@ -237,18 +237,24 @@ __device__ __forceinline__ int locate(const unsigned short *lut, const double *k
     return m;
 }
 
+// The LAST knot of an axis (x = x_max, Q^2 = q2_max) starts a phantom interval of its own: its record is
+// K1's pad entry {z_last, 1/dz = 0, 0, 0}, so t = 0 and the weights are (0, 1, 0, 0) EXACTLY -- the knot
+// reproduces its table value bit for bit, like every other knot (which is the lower knot of its own
+// interval), at no cost in the loop.  (As the upper end of the last real interval it would get
+// t = (z1 - z0) * (1 / dz), which can round to 1 - 2^-53.)  Its stencil reaches two rows / two knots past
+// the table with weight exactly 0: finite data lies there (pdfb_internal.cuh, "post").
 __device__ __forceinline__ int locate_x(const GridDev &g, const SmemViews &sv, double xv, double u)
 {
-    return locate(sv.lutx, sv.xk, g.nx - 2, xv, u, g.lutx_u0, g.lutx_inv_h);
+    return locate(sv.lutx, sv.xk, g.nx - 1, xv, u, g.lutx_u0, g.lutx_inv_h);
 }
 
 // Interval of Q^2 as an index into the CONCATENATED knot list.  A threshold is stored twice (last
 // knot of the lower sub-grid, first of the upper), so a point on it lands on the upper copy
-// (reading Q2) and the lower copy never starts an interval; only Q^2 = q2_max needs the clamp.
-// Interval records and table rows use the same index.
+// (reading Q2) and the lower copy never starts an interval; Q^2 = q2_max lands on the last knot's
+// phantom interval (above).  Interval records and table rows use the same index.
 __device__ __forceinline__ int locate_q(const GridDev &g, const SmemViews &sv, double qv, double v)
 {
-    return min(locate(sv.lutq, sv.q2k, g.nq_tot - 1, qv, v, g.lutq_v0, g.lutq_inv_h), g.nq_tot - 2);
+    return locate(sv.lutq, sv.q2k, g.nq_tot - 1, qv, v, g.lutq_v0, g.lutq_inv_h);
 }
 
 template <int W> struct YW { double v[W]; };  // one point's W columns, in column order

@@ -105,7 +105,7 @@ __device__ __forceinline__ bool xf_point_v0(const GridDev &g, const double *__re
         int i = find_interval(g.xk + xo, nxs, xv);
         IntervalRec r = load_rec(g.xrec + xo + i);
         double w[4];
-        weights4(r, (pdfb_ln(xv) - r.z0) * r.inv_dz, w);
+        weights4(r, (xv == g.x_max) ? 1.0 : (pdfb_ln(xv) - r.z0) * r.inv_dz, w);  // the last knot: t = 1 exactly (xfxq2_smem.cuh, t_coord)
         u1 = make_set(i, nxs, w);
     } else {
         rA = (pdfb_ln(xv) - g.U0) * (g.xs_per_sub ? g.inv_dU01s[s] : g.inv_dU01);
@@ -127,7 +127,7 @@ __device__ __forceinline__ bool xf_point_v0(const GridDev &g, const double *__re
         int j = find_interval(g.q2k + g.q_off[s], nq, qv);
         IntervalRec r = load_rec(g.qrec + g.q_off[s] + j);
         double w[4];
-        weights4(r, (pdfb_ln(qv) - r.z0) * r.inv_dz, w);
+        weights4(r, (qv == g.q2_max) ? 1.0 : (pdfb_ln(qv) - r.z0) * r.inv_dz, w);
         v1 = make_set(j, nq, w);
     }
     const int voff = g.v_off[s];
