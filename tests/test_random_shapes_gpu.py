@@ -57,6 +57,19 @@ def random_spec(rng):
                          np.concatenate(vals), params)
 
 
+def drop_ill_conditioned(spec, x, *others):
+    """On an x array of a handful of knots the last interval spans orders of magnitude in x while xf falls
+    to exactly 0 at x = 1: just below x = 1 the result is (1 - t) * slope with slope ~ 1, and a one-ulp
+    difference in t -- the library multiplies by a stored reciprocal, the oracle divides -- is a relative
+    1e-16 / (1 - t) on it: beyond the 1e-12 rule once 1 - t < 1e-4, for the oracle against exact arithmetic as
+    much as for the library against the oracle.  (With the >= 30 knots of real grids such results are far below
+    1e-3 and the absolute rule applies.)  Those points are left out on grids with fewer than 8 x knots."""
+    if spec.nx >= 8:
+        return (x,) + others
+    keep = (x <= 0.99) | (x == 1.0)
+    return (x[keep],) + tuple(o[keep] for o in others)
+
+
 def points(rng, spec, n_out=1500):
     x, q2 = W.scan_points(spec, per_cell=1)
     if len(x) > 6000:  # large grids: a random subset of the scan
@@ -65,7 +78,7 @@ def points(rng, spec, n_out=1500):
     x_lo = float(spec.x_knots[0])
     xo = np.exp(rng.uniform(np.log(x_lo) - 4.0, 0.0, n_out))
     qo = np.exp(rng.uniform(np.log(spec.q2_min) - 1.5, np.log(spec.q2_max) + 1.5, n_out))
-    return np.concatenate([x, xo]), np.concatenate([q2, qo])
+    return drop_ill_conditioned(spec, np.concatenate([x, xo]), np.concatenate([q2, qo]))
 
 
 @pytest.mark.parametrize("case", range(24))
@@ -109,6 +122,9 @@ def test_random_grid_shape(torch_cuda, case):
     x1 = np.exp(rng.uniform(np.log(float(spec.x_knots[0])) - 1.0, 0.0, n_ev))
     x2 = np.exp(rng.uniform(np.log(float(spec.x_knots[0])) - 1.0, 0.0, n_ev))
     qe = np.exp(rng.uniform(np.log(spec.q2_min) - 0.5, np.log(spec.q2_max) + 0.5, n_ev))
+    x1, x2, qe = drop_ill_conditioned(spec, x1, x2, qe)
+    x2, x1, qe = drop_ill_conditioned(spec, x2, x1, qe)
+    n_ev = len(x1)
     terms = [(a, b, float(rng.normal())) for a in pids for b in pids if rng.uniform() < 0.4] or [(pids[0], pids[0], 1.0)]
     lum = torch.full((n_ev,), 7.0, dtype=torch.float64, device="cuda")
     B.pdf_lumi_events(h, terms, torch.from_numpy(x1).cuda(), torch.from_numpy(x2).cuda(), torch.from_numpy(qe).cuda(), lum)
@@ -116,4 +132,94 @@ def test_random_grid_shape(torch_cuda, case):
     rl, sl = oracle.lumi_events(og, terms, x1, x2, qe, with_scale=True)
     check_parity(lum.cpu().numpy(), rl, sl, max_clause_frac=2e-2, what=f"random shape {case} lumi", log=False)
     print("case", case, shape, st)
+    B.pdf_grid_free(h)
+
+
+@pytest.mark.parametrize("case", range(16))
+def test_random_alphas_node_lists(torch_cuda, case):
+    """alpha_s on random node lists: 2 to 512 nodes (the replicated-line fast path up to 192, the general
+    kernel beyond), one to five sub-grids split by repeated nodes, sub-grids of two nodes, jittered
+    spacing, values from one-loop running times a random smooth factor.  Queries: every node, its two
+    neighbouring doubles, points inside every interval, outside the list, invalid scales; alphas_q as well."""
+    torch = torch_cuda
+    rng = np.random.default_rng(7300 + case)
+    n_sub = int(rng.integers(1, 6))
+    total = int(rng.choice([2, 3, 5, 17, 60, 100, 191, 192, 193, 300, 512]))
+    total = max(total, 2 * n_sub)
+    cuts = np.sort(rng.choice(np.arange(1, total - 1), size=n_sub - 1, replace=False)) if n_sub > 1 and total > 2 * n_sub else \
+        np.arange(2, 2 * n_sub, 2)[: n_sub - 1]
+    sizes = np.diff(np.concatenate([[0], cuts, [total]])).astype(int)
+    sizes = np.maximum(sizes, 2)
+    edges = np.exp(np.linspace(np.log(1.0), np.log(float(10.0 ** rng.uniform(2, 5))), n_sub + 1))
+    jitter = float(rng.choice([0.0, 0.2, 0.35]))
+    qs, al = [], []
+    for s in range(n_sub):
+        q = jittered_knots(rng, float(edges[s]), float(edges[s + 1]), int(sizes[s]), jitter)
+        a = W.one_loop_alphas(q * q) * (1.0 + 0.05 * s + 0.02 * np.sin(np.log(q)))
+        qs.append(q); al.append(a)
+    spec = W.AlphasSpec(np.concatenate(qs), np.concatenate(al))
+    if len(spec.q_knots) > 512:
+        pytest.skip("more than 512 nodes after padding the sub-grids")
+    oa = oracle.OracleAlphas.from_spec(spec)
+    ha = B.load_alphas_spec(spec)
+    k2 = spec.q_knots ** 2
+    mids = [np.sqrt(k2[:-1] * k2[1:]), k2[:-1] ** 0.9 * k2[1:] ** 0.1, k2[:-1] ** 0.1 * k2[1:] ** 0.9]
+    q2 = np.concatenate([k2, np.nextafter(k2, 0), np.nextafter(k2, np.inf)] + mids +
+                        [np.exp(rng.uniform(np.log(k2[0]) - 3, np.log(k2[-1]) + 3, 3000)), [0.0, -2.0, np.nan, np.inf]])
+    dq = torch.from_numpy(q2).cuda()
+    out = torch.empty_like(dq)
+    B.alphas_q2(ha, dq, out)
+    dq1 = torch.from_numpy(np.sqrt(np.where(q2 > 0, q2, np.nan))).cuda()
+    out1 = torch.empty_like(dq1)
+    B.alphas_q(ha, dq1, out1)
+    torch.cuda.synchronize()
+    ref = oa.q2(q2)
+    check_parity(out.cpu().numpy(), ref, what=f"random alpha_s list {case}: {len(k2)} nodes, sub-grids {list(sizes)}", log=False)
+    # alphas_q(Q) is alphas_q2 at Q*Q rounded once: compare with the oracle at that argument
+    qq = dq1.cpu().numpy()
+    ref1 = oa.q2(np.where(np.isnan(qq), -1.0, qq * qq))
+    check_parity(out1.cpu().numpy(), ref1, what=f"random alpha_s list {case}, Q argument", log=False)
+    B.alphas_grid_free(ha)
+
+
+@pytest.mark.parametrize("case", range(12))
+def test_random_member_sets(torch_cuda, case):
+    """PDF sets on random grid shapes: 2 to 60 members (fewer and more (member, flavour group) jobs than
+    SMs), a small batch at one scale (rows of the batch's Q^2 range only, the points' cell and t cached in
+    shared memory), a small batch over the whole Q^2 range with points outside the grid and on the last
+    knots, and a batch too large for either; member ranges; the Q-argument entry point."""
+    torch = torch_cuda
+    rng = np.random.default_rng(9100 + case)
+    spec = random_spec(rng)
+    n_mem = int(rng.choice([2, 5, 13, 40, 60]))
+    vals = np.stack([spec.values * (1.0 + 0.3 * rng.normal()) + 0.01 * rng.normal(size=spec.values.shape) * np.abs(spec.values)
+                     for _ in range(n_mem)])
+    h = B.pdf_set_load(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, vals)
+    pids = [int(p) for p in spec.pids]
+    x_lo = float(spec.x_knots[0])
+    q_one = float(np.exp(rng.uniform(np.log(spec.q2_min), np.log(spec.q2_max))))
+    batches = {
+        "one scale": (np.exp(rng.uniform(np.log(x_lo), 0.0, 1203)), np.full(1203, q_one)),
+        "top of the grid": (np.concatenate([np.exp(rng.uniform(np.log(x_lo), 0.0, 700)), [1.0, 1.0, x_lo]]),
+                            np.concatenate([np.full(700, spec.q2_max), [spec.q2_max, q_one, spec.q2_max]])),
+        "mix": points(rng, spec, n_out=800),
+        "large": (np.exp(rng.uniform(np.log(x_lo) - 1.0, 0.0, 70_001)),
+                  np.exp(rng.uniform(np.log(spec.q2_min) - 0.3, np.log(spec.q2_max) + 0.3, 70_001))),
+    }
+    for name, (x, q2) in batches.items():
+        x, q2 = drop_ill_conditioned(spec, x, q2)
+        m0 = int(rng.integers(0, n_mem))
+        cnt = int(rng.integers(1, n_mem - m0 + 1)) if name != "large" else min(2, n_mem - m0)
+        req = pids if name != "large" else pids[: min(len(pids), 5)]
+        dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+        out = torch.full((cnt, len(req), len(x)), 7.0, dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2_members(h, m0, cnt, req, dx, dq, out)
+        outq = torch.full_like(out, 7.0)
+        B.pdf_xfxq2_members(h, m0, cnt, req, dx, torch.sqrt(dq), outq, q_is_q=True)
+        torch.cuda.synchronize()
+        ref, sc = oracle.xfxq2_members(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, vals[m0:m0 + cnt], req, x, q2, with_scale=True)
+        check_parity(out.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what=f"random set {case} {name}: {n_mem} members, range {m0}+{cnt}", log=False)
+        q2r = np.sqrt(q2) ** 2  # what the Q-argument call evaluates at: Q*Q rounded once
+        refq, scq = oracle.xfxq2_members(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, vals[m0:m0 + cnt], req, x, q2r, with_scale=True)
+        check_parity(outq.cpu().numpy(), refq, scq, max_clause_frac=5e-3, what=f"random set {case} {name}, Q argument", log=False)
     B.pdf_grid_free(h)
