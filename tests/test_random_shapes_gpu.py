@@ -223,3 +223,55 @@ def test_random_member_sets(torch_cuda, case):
         refq, scq = oracle.xfxq2_members(spec.x_knots, spec.q_offsets, spec.q_knots, spec.pids, vals[m0:m0 + cnt], req, x, q2r, with_scale=True)
         check_parity(outq.cpu().numpy(), refq, scq, max_clause_frac=5e-3, what=f"random set {case} {name}, Q argument", log=False)
     B.pdf_grid_free(h)
+
+
+@pytest.mark.parametrize("case", range(8))
+def test_random_per_subgrid_x_knots_files_and_variants(torch_cuda, case, tmp_path):
+    """Sub-grids with their own x-knot arrays (different lengths and spacings on one [x_min, x_max]) on random
+    shapes, loaded directly and through a member file in the LHAPDF text layout; on the same handle the
+    fp32-output variant (= the fp64 result rounded once) and the host-buffer entry point (= the device call)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(5500 + case)
+    n_sub = int(rng.integers(2, 5))
+    nq = [int(rng.choice([2, 4, 6, 11])) for _ in range(n_sub)]
+    n_pid = int(rng.integers(1, 12))
+    pids = [int(p) for p in rng.choice(PID_POOL, size=n_pid, replace=False)]
+    x_lo = float(10.0 ** rng.uniform(-8, -3))
+    xs = [jittered_knots(rng, x_lo, 1.0, int(rng.choice([4, 9, 26, 60, 97])), float(rng.choice([0.0, 0.3]))) for _ in range(n_sub)]
+    edges = tuple(float(e) for e in np.exp(np.linspace(np.log(1.4), np.log(3e3), n_sub + 1)))
+    spec = W.make_pdf_grid_xs(xs, edges, tuple(nq), pids, seed=int(rng.integers(1, 1 << 30)))
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    h = B.load_pdf_spec(spec)
+    n = 4001
+    x = np.exp(rng.uniform(np.log(x_lo) - 2.0, 0.0, n))
+    q2 = np.exp(rng.uniform(np.log(spec.q2_min) - 1.0, np.log(spec.q2_max) + 1.0, n))
+    x[:3], q2[:3] = [1.0, x_lo, 1.0], [spec.q2_max, spec.q2_max, spec.q2_min]
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    out = torch.empty((n_pid, n), dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h, pids, dx, dq, out)
+    o32 = torch.empty((n_pid, n), dtype=torch.float32, device="cuda")
+    B.pdf_xfxq2_f32(h, pids, dx, dq, o32)
+    torch.cuda.synchronize()
+    ref, sc = og.xfxq2(pids, x, q2, with_scale=True)
+    check_parity(out.cpu().numpy(), ref, sc, max_clause_frac=5e-3, what=f"random per-sub-grid x knots {case}", log=False)
+    assert torch.equal(o32, out.to(torch.float32))
+    host = np.empty((n_pid, n))
+    B.pdf_xfxq2_host(h, pids, x, q2, host)
+    assert np.array_equal(host, out.cpu().numpy(), equal_nan=True)
+    for s in range(spec.n_sub):   # every knot of every sub-grid, bit for bit
+        q = spec.sub_q(s) if s + 1 == spec.n_sub else spec.sub_q(s)[:-1]
+        X, Q = np.meshgrid(spec.sub_x(s), q ** 2, indexing="ij")
+        ok = torch.empty((n_pid, X.size), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2(h, pids, torch.from_numpy(X.ravel().copy()).cuda(), torch.from_numpy(Q.ravel().copy()).cuda(), ok)
+        torch.cuda.synchronize()
+        assert np.array_equal(ok.cpu().numpy(), spec.sub_values(s)[:, :len(q), :].transpose(2, 0, 1).reshape(n_pid, -1)), s
+    d = tmp_path / "rset"
+    d.mkdir()
+    W.write_lhagrid(spec, str(d / "rset_0000.dat"))
+    W.write_lhapdf_info(str(d / "rset.info"), 1, pids, W.make_alphas_grid())
+    hf, ha, fp = B.load_lhapdf_set(str(d))
+    of = torch.empty_like(out)
+    B.pdf_xfxq2(hf, pids, dx, dq, of)
+    torch.cuda.synchronize()
+    assert list(fp) == pids and torch.equal(of.view(torch.int64), out.view(torch.int64))
+    B.pdf_grid_free(hf); B.alphas_grid_free(ha); B.pdf_grid_free(h)
