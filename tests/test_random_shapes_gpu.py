@@ -275,3 +275,47 @@ def test_random_per_subgrid_x_knots_files_and_variants(torch_cuda, case, tmp_pat
     torch.cuda.synchronize()
     assert list(fp) == pids and torch.equal(of.view(torch.int64), out.view(torch.int64))
     B.pdf_grid_free(hf); B.alphas_grid_free(ha); B.pdf_grid_free(h)
+
+
+@pytest.mark.parametrize("case", range(8))
+def test_random_large_mixes(torch_cuda, case):
+    """Many tiles per CTA on random shapes, with the out-of-grid share of the batch anywhere between 0 and 95 %
+    and any split between the five continuation classes: the class lists fill, trigger and flush at every
+    rhythm (a list reaching the trigger in one tile, lists that never do, all classes at once)."""
+    torch = torch_cuda
+    rng = np.random.default_rng(6600 + case)
+    while True:  # a shape the shared-memory kernel takes (every sub-grid has at least 4 Q^2 knots)
+        spec = random_spec(rng)
+        if spec.nx >= 8 and min(len(spec.sub_q(s)) for s in range(spec.n_sub)) >= 4:
+            break
+    og = oracle.OraclePdfGrid.from_spec(spec)
+    h = B.load_pdf_spec(spec)
+    assert B.pdf_grid_uses_smem_path(h)
+    pids = [int(p) for p in spec.pids]
+    n = 400_003
+    f_out = float(rng.choice([0.0, 0.02, 0.3, 0.7, 0.95]))
+    lx0, lq0, lq1 = np.log(float(spec.x_knots[0])), np.log(spec.q2_min), np.log(spec.q2_max)
+    x = np.exp(rng.uniform(lx0, 0.0, n))
+    q2 = np.exp(rng.uniform(lq0, lq1, n))
+    out_pts = rng.uniform(size=n) < f_out
+    p_cls = rng.dirichlet(np.ones(3))                      # low x | high Q | low Q (corners where two coincide)
+    kind = rng.choice(3, size=n, p=p_cls)
+    both = rng.uniform(size=n) < 0.2
+    low_x = out_pts & ((kind == 0) | both)
+    high_q = out_pts & (kind == 1)
+    low_q = out_pts & (kind == 2)
+    x[low_x] = np.exp(rng.uniform(lx0 - 6.0, lx0, int(low_x.sum())))
+    q2[high_q] = np.exp(rng.uniform(lq1, lq1 + 3.0, int(high_q.sum())))
+    q2[low_q] = np.exp(rng.uniform(lq0 - 2.0, lq0, int(low_q.sum())))
+    dx, dq = torch.from_numpy(x).cuda(), torch.from_numpy(q2).cuda()
+    out = torch.full((len(pids), n), 7.0, dtype=torch.float64, device="cuda")
+    B.pdf_xfxq2(h, pids, dx, dq, out)
+    again = torch.full_like(out, 7.0)
+    B.pdf_xfxq2(h, pids, dx, dq, again)
+    torch.cuda.synchronize()
+    assert torch.equal(out.view(torch.int64), again.view(torch.int64))
+    ref, sc = og.xfxq2(pids, x, q2, with_scale=True)
+    st = check_parity(out.cpu().numpy(), ref, sc, max_clause_frac=1e-2,
+                      what=f"random large mix {case}: nx {spec.nx}, {spec.n_pid} PIDs, {f_out:.0%} outside", log=False)
+    print("\ncase", case, spec.nx, [len(spec.sub_q(s)) for s in range(spec.n_sub)], spec.n_pid, f_out, st)
+    B.pdf_grid_free(h)
