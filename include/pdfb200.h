@@ -19,6 +19,13 @@
  *     arrays; the caller may free them immediately.
  *   - Evaluation calls with device pointers allocate nothing, never synchronise and only
  *     enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = default stream).
+ *     They can therefore be captured in a CUDA graph and replayed.
+ *   - Evaluation calls on ONE handle may be issued from several host threads and be in flight on
+ *     several streams at the same time; *_load() / *_free() / *_host() of a handle must not run
+ *     concurrently with other calls on the same handle.  (Batches of at most 65 536 points take one of
+ *     64 per-handle slots round robin: keep fewer than 64 of them in flight on one handle.)
+ *   - A given batch gives bit-identical results run to run.  A query on a knot of the grid returns
+ *     the table value bit for bit (readings O3, R-ln), the last knot of either axis included.
  *   - There is no CPU fallback: without a CUDA device *_load() fails with PDFB_ECUDA.
  */
 #ifndef PDFB200_H
