@@ -50,7 +50,9 @@ enum {
     PDFB_EXKNOTS = -8,  /* a well-formed member file / argument list this entry point cannot take:
                            sub-grids with different PID lists; or sub-grids with their own x-knot
                            arrays handed to an entry point that wants one array (use the *_xs one) */
-    PDFB_ELIMIT = -5    /* more than PDFB_MAX_SUBGRIDS subgrids or PDFB_MAX_PIDS PIDs    */
+    PDFB_ELIMIT = -5,   /* more than PDFB_MAX_SUBGRIDS subgrids or PDFB_MAX_PIDS PIDs    */
+    PDFB_ESTATIC = -9   /* alphas_q2_static: more than PDFB_STATIC_MAX_KNOTS nodes -- the node table
+                           would not fit the library's fixed scratch array; use alphas_grid_load */
 };
 #define PDFB_MAX_SUBGRIDS 16
 #define PDFB_MAX_PIDS 32
@@ -198,6 +200,43 @@ int alphas_q(const pdfb_alphas *a, long long n, const double *q, double *out, vo
 int alphas_q2_host(pdfb_alphas *a, long long n, const double *q2, double *out);
 
 void alphas_grid_free(pdfb_alphas *a);
+
+/*
+ * alphas_q2_static -- alphas_q2 for a caller that cannot allocate device memory.
+ *
+ * Who needs it.  PDFFlow runs inside a TensorFlow process, and a framework of that kind
+ * claims almost all of the GPU's memory for its own pool at start-up: a cudaMalloc issued by a side
+ * library then fails with "out of memory" however little it asks for.  The same goes for a process on
+ * a fixed device-memory quota that is already spent, and for an event loop that cannot take the
+ * device-wide synchronisation cudaMalloc / cudaFree bring.  alphas_grid_load allocates (a few KB for
+ * the node table it derives); this call does not: no cudaMalloc, no cudaFree, no allocating routine,
+ * no handle.  The derived table (ln of the nodes, interval records) goes into ONE fixed array of
+ * PDFB_STATIC_SCRATCH_BYTES (22 KB) that is part of the library image.  Every GPU of a process that
+ * loads libpdfb200.so holds that array from load to exit, used or not.
+ *
+ *   n_knots, q_knots, alphas   host arrays, the node list exactly as alphas_grid_load takes it (same
+ *                  checks, same codes).  At most PDFB_STATIC_MAX_KNOTS (256) nodes: a longer list is
+ *                  refused with PDFB_ESTATIC and nothing is launched -- load it with alphas_grid_load.
+ *   n, q2, out     device [n] on the CURRENT device (there is no handle to name one); out[i] is the
+ *                  value alphas_q2 gives (reading O6): identical bits when alphas_q2 serves the list by
+ *                  its general kernel (more than 192 nodes), within the library's 1e-12 rule when it
+ *                  serves it by the table-logarithm kernel.
+ *   cuda_stream    the node table is rebuilt on this stream ahead of the evaluation, on every call
+ *                  (3 + number of sub-grids small launches); nothing synchronises.
+ *
+ * Sharing.  All calls on a device use the same array, and it keeps whatever the previous call wrote.
+ * A call rewrites every entry it later reads, so nothing needs clearing between calls and a shorter
+ * list after a longer one is safe -- but two calls whose work overlaps on the GPU (different streams
+ * without an event between them, or two host threads) overwrite each other's table and both results
+ * are undefined.  Order them on one stream, or with events.
+ *
+ * First call.  The first call on a device looks up the array's device address (once per device, with
+ * that device current) and the SM count; make that call before starting any stream capture.
+ */
+#define PDFB_STATIC_MAX_KNOTS 256
+#define PDFB_STATIC_SCRATCH_BYTES 22528
+int alphas_q2_static(int n_knots, const double *q_knots, const double *alphas, long long n,
+                     const double *q2, double *out, void *cuda_stream);
 
 const char *pdfb_strerror(int code);
 

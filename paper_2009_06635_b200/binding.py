@@ -23,10 +23,12 @@ _ll = ctypes.c_longlong
 EXPORTS = ("pdf_grid_load", "pdf_set_load", "pdf_set_members", "pdf_xfxq2_members", "pdf_xfxq_members", "pdf_xfxq2", "pdf_xfxq", "alphas_q", "pdf_xfxq2_host", "pdf_grid_status", "pdf_grid_free",
            "alphas_grid_load", "alphas_q2", "alphas_q2_host", "alphas_grid_free", "pdfb_strerror",
            "pdfb_launch_count", "pdf_lumi_events", "pdf_xfxq2_pm", "pdf_xfxq2_f32", "pdf_grid_load_xs", "pdfb_lhagrid_dims_xs", "pdfb_lhagrid_get_xs", "pdfb_lhagrid_read", "pdfb_lhagrid_dims", "pdfb_lhagrid_get",
-           "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members")
+           "pdfb_lhagrid_free", "pdfb_lhapdf_info_alphas", "pdfb_lhapdf_info_members", "alphas_q2_static")
 
 
 PDFB_EINVAL, PDFB_EKNOTS, PDFB_EPID, PDFB_ECUDA, PDFB_ELIMIT, PDFB_EIO, PDFB_EFORMAT, PDFB_EXKNOTS = -1, -2, -3, -4, -5, -6, -7, -8
+PDFB_ESTATIC = -9
+PDFB_STATIC_MAX_KNOTS = 256
 
 
 class PdfbError(RuntimeError):
@@ -82,6 +84,8 @@ def lib():
         L.alphas_q2.argtypes = [_vp, _ll, _vp, _vp, _vp]
         L.alphas_q2_host.restype = ctypes.c_int
         L.alphas_q2_host.argtypes = [_vp, _ll, _vp, _vp]
+        L.alphas_q2_static.restype = ctypes.c_int
+        L.alphas_q2_static.argtypes = [ctypes.c_int, _dp, _dp, _ll, _vp, _vp, _vp]
         L.alphas_grid_free.restype = None
         L.alphas_grid_free.argtypes = [_vp]
         L.pdfb_strerror.restype = ctypes.c_char_p
@@ -349,6 +353,20 @@ def alphas_q2_host(a, q2, out):
     n = int(q2.size if isinstance(q2, np.ndarray) else q2.numel())
     rc = lib().alphas_q2_host(_vp(a), n, _host_ptr(q2, n, "q2"), _host_ptr(out, n, "out"))
     _check(rc, "alphas_q2_host")
+
+
+def alphas_q2_static(q_knots, alphas, q2, out, stream=None, n=None):
+    """alpha_s(Q^2) without a handle and without any device allocation (include/pdfb200.h): for use
+    inside a process whose framework owns the GPU's memory pool, where the library's own cudaMalloc
+    would fail.  q_knots / alphas: host node list of at most PDFB_STATIC_MAX_KNOTS nodes; q2 / out:
+    torch CUDA tensors on the current device.  Calls that overlap on the GPU race on the shared table."""
+    q_knots, alphas = _f64(q_knots), _f64(alphas)
+    if q_knots.shape != alphas.shape:
+        raise ValueError("q_knots and alphas differ in length")
+    n = int(q2.numel() if n is None else n)
+    rc = lib().alphas_q2_static(len(q_knots), q_knots.ctypes.data_as(_dp), alphas.ctypes.data_as(_dp), n,
+                                _dev_ptr(q2, n, "q2"), _dev_ptr(out, n, "out"), _stream_ptr(stream))
+    _check(rc, "alphas_q2_static")
 
 
 def alphas_grid_free(a):

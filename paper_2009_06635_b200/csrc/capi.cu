@@ -25,6 +25,7 @@ extern "C" const char *pdfb_strerror(int code)
     case PDFB_EFORMAT: return "file is not in the expected LHAPDF text layout";
     case PDFB_EXKNOTS: return "sub-grids with different PID lists, or sub-grids with their own x-knot arrays passed to an entry point that takes one array (use pdf_grid_load_xs / pdfb_lhagrid_*_xs)";
     case PDFB_ELIMIT: return "too many sub-grids, PIDs or alpha_s nodes";
+    case PDFB_ESTATIC: return "alphas_q2_static takes at most 256 nodes (PDFB_STATIC_MAX_KNOTS): the node table must fit the library's fixed scratch array; load longer lists with alphas_grid_load";
     default: return "unknown pdfb error code";
     }
 }

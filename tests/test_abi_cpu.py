@@ -91,3 +91,21 @@ def test_null_handles_rejected(L):
     assert rc == -1
     rc = L.alphas_q2(None, 0, None, None, None)
     assert rc == -1
+
+
+def test_alphas_q2_static_validates_before_cuda(L):
+    """The no-allocation entry point checks its node list on the host, before any CUDA call: a list
+    longer than its fixed scratch array holds is refused with a code of its own."""
+    qk = np.geomspace(1.0, 1e4, B.PDFB_STATIC_MAX_KNOTS + 1)
+    al = np.linspace(0.3, 0.1, len(qk))
+    dp = ctypes.POINTER(ctypes.c_double)
+    rc = L.alphas_q2_static(len(qk), qk.ctypes.data_as(dp), al.ctypes.data_as(dp), 0, None, None, None)
+    assert rc == B.PDFB_ESTATIC and "256" in B.strerror(rc)
+    qk, al = qk[:-1].copy(), al[:-1].copy()
+    assert L.alphas_q2_static(len(qk), qk.ctypes.data_as(dp), al.ctypes.data_as(dp), 0, None, None, None) == 0   # n = 0: nothing to do
+    assert L.alphas_q2_static(len(qk), qk.ctypes.data_as(dp), al.ctypes.data_as(dp), 5, None, None, None) == B.PDFB_EINVAL
+    assert L.alphas_q2_static(1, qk.ctypes.data_as(dp), al.ctypes.data_as(dp), 0, None, None, None) == B.PDFB_EINVAL
+    qk[7] = qk[6] * 0.5
+    assert L.alphas_q2_static(len(qk), qk.ctypes.data_as(dp), al.ctypes.data_as(dp), 0, None, None, None) == B.PDFB_EKNOTS
+    hdr = open(os.path.join(ROOT, "include", "pdfb200.h")).read()
+    assert f"#define PDFB_STATIC_MAX_KNOTS {B.PDFB_STATIC_MAX_KNOTS}" in hdr
