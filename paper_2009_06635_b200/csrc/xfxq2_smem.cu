@@ -61,7 +61,12 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
     const int lo = r0 * RBs, stage = (r1 - r0) * RBs;
     int shift = 0;
     if (SETS && row_range) {
-        const int rows = (r1 - r0 + 1) & ~1;  // even: the copy keeps the bank alignment of 2-column rows
+        // even: the copy keeps the bank alignment of 2-column rows.  With r0 == 0 the stencils of Q^2
+        // intervals 0 and 1 reach below row 0 with weight exactly 0: row -1, and (x interval 0 of Q^2
+        // interval 0: knot -1 of row -1) the tail of row -2.  For buffer 0 that is the tail of `pre`;
+        // for buffer 1 it is what lies below its row 0 -- so two rows are left free between the two
+        // buffers there and zero-filled below (no bulk copy ever writes them).
+        const int rows = (r1 - r0 + (r0 == 0 ? 3 : 1)) & ~1;
         if ((rows + r1) * RBs <= slice_bytes) shift = rows * RBs;
     }
     auto stage_job = [&](int j, int buf) {  // one thread: the rows of job j into buffer buf
@@ -95,6 +100,10 @@ k_xfxq2_smem(const __grid_constant__ GridDev g, const __grid_constant__ PassList
 #endif
     __syncthreads();
     if (tid == 0) stage_job(job, 0);
+    if (SETS && shift && r0 == 0) {  // the two free rows below buffer 1 (see `rows` above): finite data for zero-weight reads
+        for (int e = tid; e < 2 * RBs / 16; e += NT_SMEM)
+            asm volatile("st.shared.v4.u32 [%0], {%1, %1, %1, %1};" ::"r"(tab0 + (uint32_t)(shift - 2 * RBs + e * 16)), "r"(0) : "memory");
+    }
     {   // pre and post blocks around the slice (both multiples of 128 bytes)
         const int4 *src = reinterpret_cast<const int4 *>(g.aux);
         int4 *pre = reinterpret_cast<int4 *>(smem), *post = reinterpret_cast<int4 *>(smem + g.pre_bytes + slice_bytes);

@@ -355,6 +355,46 @@ def test_member_set(torch_cuda):
     B.pdf_grid_free(ht)
 
 
+def test_member_set_low_q2_rows_double_buffered(torch_cuda):
+    """More jobs than SMs on a small batch whose Q^2 values sit in the FIRST intervals of the table: the
+    set kernel stages rows 0.. twice (one copy per in-flight job), and the stencils of Q^2 intervals 0
+    and 1 reach the row below row 0 with weight exactly 0 -- also in the second copy, where that row is
+    not the block in front of the slice.  x includes the first x interval (knot -1 of a row = the tail
+    of the row below).  Whatever is read there must be finite: every member equals the oracle, no NaN;
+    under the poisoned build (-DPDFB_CHECKED) an unstaged read shows up as NaN."""
+    torch = torch_cuda
+    n_mem = 60                                   # 240 jobs > 148 SMs: persistent CTAs, next job's rows in flight
+    g0 = W.grid_member(0)
+    vals = W.member_values(n_mem)
+    h = B.pdf_set_load(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals)
+    assert B.pdf_grid_uses_smem_path(h)
+    pids = list(W.PIDS_13)
+    q2k = np.asarray(g0.q_knots[:4], dtype=np.float64) ** 2
+    rng = np.random.Generator(np.random.PCG64(4242))
+    n = 3001
+    x = np.exp(rng.uniform(np.log(g0.x_knots[0]), np.log(g0.x_knots[-1]), n))
+    x[:600] = np.exp(rng.uniform(np.log(g0.x_knots[0]), np.log(g0.x_knots[1]), 600))   # first x interval
+    x[0], x[1] = g0.x_knots[0], g0.x_knots[1]
+    x = np.clip(x, g0.x_knots[0], g0.x_knots[-1])
+    cases = {
+        "interval 1 only": np.exp(rng.uniform(np.log(q2k[1]), np.log(q2k[2]), n)).clip(q2k[1], q2k[2] * (1 - 1e-12)),
+        "intervals 0 and 1": np.exp(rng.uniform(np.log(q2k[0]), np.log(q2k[2]), n)).clip(q2k[0], q2k[2] * (1 - 1e-12)),
+        "interval 0 only": np.exp(rng.uniform(np.log(q2k[0]), np.log(q2k[1]), n)).clip(q2k[0], q2k[1] * (1 - 1e-12)),
+        "intervals 1 and 2": np.exp(rng.uniform(np.log(q2k[1]), np.log(q2k[3]), n)).clip(q2k[1], q2k[3] * (1 - 1e-12)),
+    }
+    dx = torch.from_numpy(x).cuda()
+    for name, q2 in cases.items():
+        dq = torch.from_numpy(q2).cuda()
+        out = torch.empty((n_mem, len(pids), n), dtype=torch.float64, device="cuda")
+        B.pdf_xfxq2_members(h, 0, n_mem, pids, dx, dq, out)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert np.isfinite(got).all(), name
+        ref, sc = oracle.xfxq2_members(g0.x_knots, g0.q_offsets, g0.q_knots, g0.pids, vals, pids, x, q2, with_scale=True)
+        check_parity(got, ref, sc, what="member set, low rows: " + name)
+    B.pdf_grid_free(h)
+
+
 def test_set_loaded_from_lhapdf_layout_files(torch_cuda, tmp_path):
     """A synthetic set written in the LHAPDF6 text layout (3 member files + metadata with the alpha_s
     nodes) and loaded through the front-end evaluates bit-identically to the same arrays loaded
