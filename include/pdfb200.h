@@ -23,7 +23,10 @@
  *   - Evaluation calls on ONE handle may be issued from several host threads and be in flight on
  *     several streams at the same time; *_load() / *_free() / *_host() of a handle must not run
  *     concurrently with other calls on the same handle.  (Batches of at most 65 536 points take one of
- *     64 per-handle slots round robin: keep fewer than 64 of them in flight on one handle.)
+ *     64 per-handle slots round robin: keep fewer than 64 of them in flight on one handle.  A call that
+ *     is recorded by a stream capture takes its slot from a second ring of 64 that live calls never
+ *     use, and keeps it for every replay: a graph may replay next to any live calls, and one handle
+ *     serves up to 64 recorded small-batch calls that can run at the same time.)
  *   - A given batch gives bit-identical results run to run.  A query on a knot of the grid returns
  *     the table value bit for bit (readings O3, R-ln), the last knot of either axis included.
  *   - There is no CPU fallback: without a CUDA device *_load() fails with PDFB_ECUDA.

@@ -93,6 +93,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
 
     pdfb_grid *g = new (std::nothrow) pdfb_grid();
     if (!g) return PDFB_EINVAL;
+    g->rr_cap_next.store(0);
     g->rr_next.store(0);  // (new pdfb_grid() value-initialises: every other member is zero)
     g->device = device;
     if (cudaDeviceGetAttribute(&g->sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { delete g; return PDFB_ECUDA; }
@@ -160,7 +161,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     size_t o_valg2 = align_up(o_valg + (size_t)d.slice_bytes * d.n_groups * n_g4, 128);
     size_t o_aux = align_up(o_valg2 + (size_t)d.slice2_bytes * d.n_groups2 * n_g2, 128);
     size_t o_rr = align_up(o_aux + aux_bytes, 128);
-    size_t o_ws = align_up(o_rr + sizeof(int) * 2 * PDFB_RR_SLOTS, 128);
+    size_t o_ws = align_up(o_rr + sizeof(int) * 2 * (PDFB_RR_SLOTS + PDFB_RR_CAP_SLOTS), 128);
     size_t total = o_ws + PDFB_WS_BYTES;
     char *blob = nullptr, *raw = nullptr;
     const long long member_values = knots * n_pid;  // doubles of one member in file order

@@ -59,6 +59,7 @@ extern "C" int pdf_grid_load_xs(int n_sub, const int *x_offsets, const double *x
     if (!guard.ok) return PDFB_ECUDA;
     pdfb_grid *g = new (std::nothrow) pdfb_grid();
     if (!g) return PDFB_EINVAL;
+    g->rr_cap_next.store(0);
     g->rr_next.store(0);  // (new pdfb_grid() value-initialises: every other member is zero)
     g->device = device;
     if (cudaDeviceGetAttribute(&g->sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) { delete g; return PDFB_ECUDA; }

@@ -155,7 +155,7 @@ struct GridDev {
     const IntervalRec *qrec;           // [nq_tot]; entry q_off[s]+j = interval j of sub-grid s
     const double *val;                 // [member][s][iq][ix][kpad]: knot (s,ix,iq) at v_off[s]+iq*nx+ix
     unsigned long long *n_invalid;     // sticky counter
-    int *row_range;                    // smem path: PDFB_RR_SLOTS x {first row, end row} staged by a small-batch call (xfxq2_smem.cu)
+    int *row_range;                    // smem path: (PDFB_RR_SLOTS + PDFB_RR_CAP_SLOTS) x {first row, end row} staged by a small-batch call (xfxq2_smem.cu)
     uint32_t *slow_ws;                 // smem path: per SM and warp, PDFB_SLOW_CLASSES lists of out-of-grid point indices
     // ---- shared-memory path (xfxq2_smem.cu): flavour-group slices + a small aux block
     int smem_ok;                       // bit 0: the 4-column slices fit shared memory; bit 1: the 2-column ones
@@ -178,6 +178,8 @@ struct GridDev {
 #define PDFB_LUT_BINS 512
 #endif
 #define PDFB_RR_SLOTS 64      // row-range slots of a handle: calls in flight on one handle that may use one each
+#define PDFB_RR_CAP_SLOTS 64  // ... and as many again that only calls recorded by a stream capture take: a recorded call
+                              // keeps its slot for every replay of its graph, so it must not sit in the live calls' ring
 #define PDFB_SLOW_CLASSES 5   // x < x_min | Q^2 > max | Q^2 < min | the two corners
 #define PDFB_WS_SLOTS 160     // >= %nsmid (148 on B200; checked at load): one scratch slot per SM
 #ifndef PDFB_SLOW_TRIGGER
@@ -244,6 +246,7 @@ struct pdfb_grid {
     int device;
     int sms;                  // multiprocessors of `device`
     std::atomic<unsigned> rr_next;  // next row-range slot (round robin)
+    std::atomic<unsigned> rr_cap_next;  // next row-range slot of a call recorded by a stream capture
     LumiLayout lumi;          // band plan of pdf_lumi_events
     int lumi_npair;           // its kernel instance (column pairs staged per band); 0 = general kernel only
     GridDev d;

@@ -453,7 +453,16 @@ int pdfb_launch_xfxq2_smem(const pdfb_grid *g, int n_req, const int *cols, long 
     // small batch on a big slice: find the rows it needs first (one more launch of a single CTA)
     const int *rr = nullptr;
     if (n <= PDFB_RR_MAX_POINTS && (W == 4 ? g->d.slice_bytes : g->d.slice2_bytes) >= PDFB_RR_MIN_SLICE) {
-        int *slot = g->d.row_range + 2 * (const_cast<pdfb_grid *>(g)->rr_next.fetch_add(1, std::memory_order_relaxed) % PDFB_RR_SLOTS);
+        // A call recorded by a stream capture keeps the slot chosen here for every replay of its graph: it
+        // takes one from a ring of its own, which live calls never use (a replay running next to any
+        // number of live calls cannot meet one of them in a slot).
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cap) != cudaSuccess) { cudaGetLastError(); cap = cudaStreamCaptureStatusNone; }  // (legacy stream next to a capture)
+        pdfb_grid *gm = const_cast<pdfb_grid *>(g);
+        const unsigned idx = (cap == cudaStreamCaptureStatusActive)
+                                 ? PDFB_RR_SLOTS + gm->rr_cap_next.fetch_add(1, std::memory_order_relaxed) % PDFB_RR_CAP_SLOTS
+                                 : gm->rr_next.fetch_add(1, std::memory_order_relaxed) % PDFB_RR_SLOTS;
+        int *slot = g->d.row_range + 2 * idx;
         if (mode & 1) k_row_range<true><<<1, 1024, 0, st>>>(g->d, n, x, q2, slot);
         else k_row_range<false><<<1, 1024, 0, st>>>(g->d, n, x, q2, slot);
         pdfb_count_launch(1);

@@ -182,6 +182,47 @@ def test_calls_can_be_captured_in_a_cuda_graph(torch_cuda, grid2, ograph2, h2):
     B.alphas_grid_free(ha)
 
 
+def test_graph_replay_next_to_live_small_batches(torch_cuda, grid2, h2):
+    """A small batch first asks a one-CTA pre-pass which table rows it needs; the answer sits in a
+    per-handle slot.  A call recorded into a CUDA graph keeps its slot for every replay, so recorded calls
+    take theirs from a ring that live calls never use (xfxq2_smem.cu): a graph replaying on one stream
+    while hundreds of live small batches -- on other table rows -- go through the live ring on another
+    stream still gives, bit for bit, what the same call gives alone; so does every live call."""
+    torch = torch_cuda
+    pids = list(W.PIDS_11)
+    n_s = 2_003
+    rng = np.random.Generator(np.random.PCG64(99))
+    q2k = np.asarray(grid2.q_knots, dtype=np.float64) ** 2
+    x = np.exp(rng.uniform(np.log(grid2.x_knots[0]), np.log(grid2.x_knots[-1]), n_s)).clip(grid2.x_knots[0], grid2.x_knots[-1])
+    q_lo = np.exp(rng.uniform(np.log(q2k[1]), np.log(q2k[3]), n_s)).clip(q2k[1], q2k[3])          # bottom rows
+    q_hi = np.exp(rng.uniform(np.log(q2k[-4]), np.log(q2k[-2]), n_s)).clip(q2k[-4], q2k[-2])      # top rows
+    dx, dlo, dhi = (torch.from_numpy(a).cuda() for a in (x, q_lo, q_hi))
+    want_lo = torch.empty((len(pids), n_s), dtype=torch.float64, device="cuda")
+    want_hi = torch.empty_like(want_lo)
+    B.pdf_xfxq2(h2, pids, dx, dlo, want_lo)
+    B.pdf_xfxq2(h2, pids, dx, dhi, want_hi)
+    torch.cuda.synchronize()
+    side, live = torch.cuda.Stream(), torch.cuda.Stream()
+    o_g = torch.empty_like(want_lo)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        B.pdf_xfxq2(h2, pids, dx, dlo, o_g)
+    n_live = 40
+    o_live = [torch.empty_like(want_hi) for _ in range(n_live)]
+    for rnd in range(12):                          # 480 live calls: the live ring wraps seven times
+        o_g.fill_(float("nan"))
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            for _ in range(20):
+                graph.replay()
+        for o in o_live:
+            B.pdf_xfxq2(h2, pids, dx, dhi, o, stream=live)
+        torch.cuda.synchronize()
+        assert torch.equal(o_g.view(torch.int64), want_lo.view(torch.int64)), rnd
+        for o in o_live:
+            assert torch.equal(o.view(torch.int64), want_hi.view(torch.int64)), rnd
+
+
 def test_more_than_2_to_the_31_points(torch_cuda, grid2, ograph2, h2):
     """Maximum sizes: the class lists hold point indices as 32-bit offsets, so a batch beyond 2^31 points
     goes out in slices of 2^31 (xfxq2_smem.cu).  2^31 + 70 001 points, PID 21, a fifth of them below
