@@ -85,7 +85,7 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
     auto eval = [&](double qv) -> double {
         double res;
         if (Q_IS_Q) qv = (qv > 0.0) ? qv * qv : -1.0;  // Q in GeV -> Q^2
-        if (qv >= A.q2_min && qv <= A.q2_max) {
+        if (qv >= A.q2_min && qv < A.q2_max) {  // (Q^2 = the last node takes the frozen branch: the node value, bit for bit)
             double2 le;  // {1/c, ln c} of qv's mantissa bin
             asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(le.x), "=d"(le.y) : "r"(lntab + (uint32_t)ln_tab_bin(qv) * 128u));
             const double v = ln_tab(qv, le);
@@ -95,7 +95,7 @@ k_alphas_fast(const __grid_constant__ AlphasDev A, long long n, const double *__
             if (d) { if (q2k[m + d] <= qv) m += d; }
             if (e & 1)
                 while (m < A.K - 1 && q2k[m + 1] <= qv) ++m;
-            m = min(m, A.K - 2);  // Q^2 = last node: last interval, t = 1
+            m = min(m, A.K - 2);
             const uint32_t rec = lines + (uint32_t)m * (uint32_t)PDFB_ALPHAS_LINE;
             double2 zd, d12;
             double d3;

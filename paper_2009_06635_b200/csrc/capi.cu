@@ -173,7 +173,7 @@ extern "C" int pdf_set_load(int n_members, int n_sub, int nx, const double *x_kn
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
         if (e0) cudaEventDestroy(e0);
-        cudaFree(blob); delete g;
+        cudaFree(raw); cudaFree(blob); delete g;
         return PDFB_ECUDA;
     }
     do {

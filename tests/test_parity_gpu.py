@@ -139,6 +139,25 @@ def test_alphas_edges_thresholds_and_outside(torch_cuda):
     B.alphas_grid_free(ha)
 
 
+@pytest.mark.parametrize("n_nodes", [100, 240])  # table-logarithm kernel (<= 192 nodes) and the general one
+def test_alphas_on_a_node_is_the_node_value(torch_cuda, n_nodes):
+    """include/pdfb200.h: a query on a knot returns the table value bit for bit -- for alpha_s too, in
+    both kernels, the LAST node included (at a flavour threshold, stored twice, the upper copy)."""
+    per = n_nodes // 4
+    aspec = W.make_alphas_grid(nq_per_sub=(per, per, per, n_nodes - 3 * per), jump=(1.0, 1.02, 1.0404, 1.061208))
+    ha = B.load_alphas_spec(aspec)
+    k2 = aspec.q_knots ** 2
+    dq = torch_cuda.from_numpy(k2).cuda()
+    out = torch_cuda.empty_like(dq)
+    B.alphas_q2(ha, dq, out)
+    torch_cuda.cuda.synchronize()
+    want = aspec.alphas.copy()
+    rep = np.nonzero(k2[1:] == k2[:-1])[0]          # lower copy of a threshold: the query lands on the upper one
+    want[rep] = aspec.alphas[rep + 1]
+    assert np.array_equal(out.cpu().numpy(), want)
+    B.alphas_grid_free(ha)
+
+
 def test_invalid_points_nan_and_counted(torch_cuda, grid1):
     h = B.load_pdf_spec(grid1)
     x = np.array([0.5, 1.0000001, 0.0, -0.1, np.nan, 0.5, 0.5, 0.5, np.inf, 0.5])
