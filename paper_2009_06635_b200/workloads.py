@@ -360,9 +360,10 @@ def scan_points(grid: PdfGridSpec, per_cell: int = 3):
 # --------------------------------------------------------------------------
 def write_lhagrid(spec: PdfGridSpec, path: str, pdf_type: str = "central", x_knots_per_sub=None) -> None:
     """Member file in the LHAPDF6 text layout.  ``x_knots_per_sub`` (a list of x-knot arrays, one per
-    sub-grid) writes a file whose sub-grids carry DIFFERENT x knots -- legal in LHAPDF, refused by
-    this library with PDFB_EXKNOTS; the values of such a block are the analytic family of
-    ``spec.params`` on those knots (the file is for reader tests)."""
+    sub-grid) writes a file whose sub-grids carry DIFFERENT x knots -- legal in LHAPDF; the library
+    reads such a file with pdfb_lhagrid_dims_xs / _get_xs and loads it with pdf_grid_load_xs (the
+    one-array entry points pdfb_lhagrid_dims / _get answer PDFB_EXKNOTS); the values of such a block
+    are the analytic family of ``spec.params`` on those knots."""
     r = lambda a: " ".join(repr(float(v)) for v in a)
     with open(path, "w") as f:
         f.write(f"PdfType: {pdf_type}\nFormat: lhagrid1\n---\n")
