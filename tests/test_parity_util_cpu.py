@@ -40,3 +40,16 @@ def test_rule_and_clause(grid2, ograph2, tmp_path, monkeypatch):
     assert tot["n"] == int((~np.isnan(ref)).sum()) and tot["n_clause"] == 0
     lines = (tmp_path / "log.jsonl").read_text().strip().splitlines()
     assert len(lines) >= 4 and '"what": "pop"' in lines[-1]
+
+
+def test_slack_is_added_to_the_rule_only_where_given():
+    """check_parity(slack=...): an output beyond the 1e-12 / 1e-15 rule passes iff the caller's derived
+    allowance covers the excess; outputs with zero slack stay under the plain rule; uses are counted."""
+    ref = np.array([[1.0, 2.0, 1e-6, 3.0]])
+    got = ref + np.array([[5e-12, 0.0, 4e-15, 1e-13]])
+    with pytest.raises(AssertionError):
+        check_parity(got, ref, what="no slack", log=False)
+    st = check_parity(got, ref, what="slack", log=False, slack=np.array([[5e-12, 0.0, 4e-15, 0.0]]))
+    assert st["n_slack"] == 2 and st["n_clause"] == 0 and 0.7 < st["max_slack_used"] < 1.3   # (|d| / slack; the rule itself comes on top)
+    with pytest.raises(AssertionError):   # the slack sits on the wrong outputs
+        check_parity(got, ref, what="misplaced", log=False, slack=np.array([[0.0, 5e-12, 0.0, 4e-15]]))
