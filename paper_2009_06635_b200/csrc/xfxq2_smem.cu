@@ -368,11 +368,36 @@ static const int STATIC_SMEM = 256;  // >= the kernel's static shared memory (mb
 static_assert(NT_SMEM == 512, "PDFB_WS_BYTES and the request flags assume 16 warps per CTA");
 static_assert(PDFB_SLOW_TRIGGER - 1 + 32 + 31 <= 255 && PDFB_SLOW_TRIGGER + 62 <= PDFB_SLOW_LCAP, "8-bit list counters");
 
+// %nsmid as the device itself reports it: the class-list scratch is indexed by %smid, and PTX promises
+// %smid < %nsmid, not %smid < the SM count of the runtime's device properties.
+static __device__ unsigned g_nsmid;
+__global__ void k_read_nsmid()
+{
+    unsigned v;
+    asm("mov.u32 %0, %%nsmid;" : "=r"(v));
+    g_nsmid = v;
+}
+static int device_nsmid(int device)  // the caller has made `device` current (pdf_set_load); -1 on error
+{
+    static std::atomic<int> cached[64];
+    if (device < 0 || device >= 64) return -1;
+    int v = cached[device].load(std::memory_order_acquire);
+    if (v > 0) return v;
+    unsigned h = 0;
+    k_read_nsmid<<<1, 1>>>();
+    pdfb_count_launch(1);
+    if (cudaMemcpyFromSymbol(&h, g_nsmid, sizeof(h)) != cudaSuccess || h == 0) { cudaGetLastError(); return -1; }
+    cached[device].store((int)h, std::memory_order_release);
+    return (int)h;
+}
+
 // bit 0: the 4-column slices fit the device's shared memory, bit 1: the 2-column slices do
 int pdfb_smem_eligible(const pdfb_grid *g)
 {
     if (getenv("PDFB_FORCE_FALLBACK")) return 0;  // testing: force the read-only-cache path
-    if (g->sms > PDFB_WS_SLOTS) return 0;         // one scratch slot per SM (%smid < %nsmid = the SM count)
+    if (g->sms > PDFB_WS_SLOTS) return 0;         // one scratch slot per SM ...
+    const int nsmid = device_nsmid(g->device);    // ... indexed by %smid < %nsmid (read from the device, not assumed = the SM count)
+    if (nsmid < 1 || nsmid > PDFB_WS_SLOTS) return 0;
     int dev_max = 0;
     if (cudaDeviceGetAttribute(&dev_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, g->device) != cudaSuccess) return 0;
     int ok = 0;
