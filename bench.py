@@ -22,15 +22,26 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2009_06635_b200 import workloads as W  # noqa: E402
+from paper_2009_06635_b200 import sharding, workloads as W  # noqa: E402
 
 METRIC = "pdf_evaluations_per_sec"
 UNIT = "evaluations/s"
 N_FULL = 100_000_000
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_xfxq2_smem launch at 1e8 points x 11
-# flavours, from the `ncu --set full` capture summarised in profiles/r2_kernels.md
-NCU_TRAFFIC_BYTES_PER_POINT = (1.612596e9 + 8.742418e9) / 1e8
-NCU_TRAFFIC_SOURCE = "profiles/r2_kernels.md (ncu --set full, 1e8 points; scaled by points)"
+
+
+def ncu_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_xfxq2_smem launch on the config-3 batch, per
+    point, read from profiles/r3_traffic.json -- the file the `ncu --set full` capture of that launch is
+    turned into (command in profiles/r3_traffic.md).  None if the file is missing: a stale literal in
+    this source would not notice a regression, a missing capture is visible."""
+    p = os.path.join(ROOT, "profiles", "r3_traffic.json")
+    try:
+        with open(p) as f:
+            t = json.load(f)
+        return (float(t["dram_bytes_read"]) + float(t["dram_bytes_write"])) / float(t["points"]), \
+            f"profiles/r3_traffic.json ({t.get('source', 'ncu --set full')}; scaled by points)"
+    except (OSError, ValueError, KeyError):
+        return None, "profiles/r3_traffic.json missing"
 
 
 def measured_peaks():
@@ -114,6 +125,39 @@ def cpu_baseline(grid, x, q2, pids, target_s=12.0):
             "sample": f"first {m} points of the config-3 batch x {len(pids)} flavours, {dt:.1f} s",
             "value_1_thread": m1 * len(pids) / dt1, "sample_1_thread": f"first {m1} points, {dt1:.1f} s",
             "note": "oracle ln = binary128 logq rounded once (reading R-ln): slower than a libm-log oracle"}
+
+
+def cpu_baseline_other_configs(grid, target_s=2.0):
+    """The oracle as it stands on the first points of configs 1, 2, 4 and 5 ("on the first
+    min(N, 1e7) points of each of the five configs", one thread and all cores) -- bounded to about
+    `target_s` seconds per config and thread count so that the default run stays within minutes; the
+    sample is stated.  Evaluations (points x flavours) per second."""
+    import oracle
+    cores = oracle.threads()
+    p11 = list(W.PIDS_11)
+    g1 = W.grid_config1()
+    x1, x2, qe = W.queries_mc_events(grid, 10_000_000)
+    cases = {
+        "config1_1e4x3": (oracle.OraclePdfGrid.from_spec(g1), list(W.PIDS_3), 10_000) + W.queries_in_range(g1, 10_000, 1),
+        "config2_1e6x11": (oracle.OraclePdfGrid.from_spec(grid), p11, 1_000_000) + W.queries_in_range(grid, 1_000_000, 2),
+        "config4_mix_1e7x11": (oracle.OraclePdfGrid.from_spec(grid), p11, 10_000_000) + W.queries_extrapolation_mix(grid, 10_000_000),
+        "config5_1e7_events": (oracle.OraclePdfGrid.from_spec(grid), p11, 10_000_000, x1, qe),
+    }
+    res = {}
+    for name, (og, pids, n_full, x, q2) in cases.items():
+        e = {"unit": UNIT, "kind": "oracle", "cores": cores}
+        for threads, key in ((cores, "value"), (1, "value_1_thread")):
+            oracle.set_threads(threads)
+            m = min(n_full, 20_000)
+            t = time.perf_counter(); og.xfxq2(pids, x[:m], q2[:m]); rate = m / (time.perf_counter() - t)
+            m = int(min(n_full, max(m, rate * target_s)))
+            t = time.perf_counter(); og.xfxq2(pids, x[:m], q2[:m]); dt = time.perf_counter() - t
+            e[key] = m * len(pids) / dt
+            e["sample" if threads != 1 else "sample_1_thread"] = f"first {m} of {n_full} points x {len(pids)} flavours, {dt:.1f} s"
+        oracle.set_threads(cores)
+        res[name] = e
+    res["config5_1e7_events"]["note"] = "the x1 leg of the events (the x2 leg and alpha_s cost the oracle the same per point / far less)"
+    return res
 
 
 def parity_population(torch, out_d, grid, x_h, q2_h, pids, chunk=10_000_000):
@@ -288,7 +332,7 @@ def bench_other_configs(torch, B, h, ha, grid, peak, fma_per_s, graph=True):
     return res
 
 
-def bench_members(torch, B, local, n_rep):
+def bench_members(torch, B, local, n_rep, hbm_gbs=None, lds_bps=None, fma_per_s=None):
     """SURVEY.md 8(f).1 / PAPER.md:171-190, Table 2: all 13 flavours of N_rep members on a 2415-point
     x-grid, one pdf_xfxq2_members launch; reported beside the metric, not inside it."""
     g0 = W.grid_member(0)
@@ -308,11 +352,30 @@ def bench_members(torch, B, local, n_rep):
     ms = a.elapsed_time(b) / 10
     B.pdf_grid_free(hs)
     ev = n_rep * len(pids) * len(x)
-    # the slices are read once from HBM (the set does not fit L2 at N_rep = 400), the outputs written once
-    bytes_alg = n_rep * 4 * 100 * 64 * 32 + 8 * ev
+    # Algorithmic traffic of the launch: all points sit at the grid's lowest scale, so a member's stencils
+    # touch table rows 0..3 of the 64 (rows -1..2 of Q^2 interval 0 plus the head of row 3) in each of its
+    # 4 flavour-group slices -- 4 rows x 100 knots x 32 B -- read once; the points are read once per job
+    # (L2-resident after the first), the outputs written once.
+    n_groups, rows_needed, row_bytes = 4, 4, 100 * 32
+    bytes_alg = n_rep * n_groups * rows_needed * row_bytes + 16 * len(x) + 8 * ev
+    t = ms * 1e-3
+    roof = None
+    if hbm_gbs and lds_bps and fma_per_s:
+        # three bounds of one launch: HBM on the algorithmic bytes, the on-chip stencil gather (one 4-column
+        # group = 128 B x 4 rows per point: 16 LDS.128; 4 groups hold 13 + 3 padding columns) and FP64
+        # (per job and point: two weight sets from the cached t, tau ~ 40 FMA, 4 x 20 contraction)
+        t_hbm = bytes_alg / (hbm_gbs * 1e9)
+        gather_bytes = n_rep * n_groups * len(x) * 4 * 128
+        t_gather = gather_bytes / lds_bps
+        t_fp64 = n_rep * n_groups * len(x) * (40 + 80) / fma_per_s
+        b = max((t_gather, "smem"), (t_hbm, "hbm"), (t_fp64, "alu"))
+        roof = {"bound": b[1], "frac": b[0] / t, "roofline_ms": b[0] * 1e3, "hbm_frac": t_hbm / t, "smem_frac": t_gather / t,
+                "fp64_frac": t_fp64 / t, "achieved": gather_bytes / t / 1e9, "peak": lds_bps / 1e9, "unit": "GB/s",
+                "peak_source": "measured: pdfb_probe(PDFB_PROBE_LDS), conflict-free LDS.128",
+                "note": "the launch moves 0.06 of a slice per job, so the stencil gather from shared memory, not HBM, bounds it"}
     paper = {10: 0.07, 50: 0.35, 100: 0.69, 200: 1.46, 300: 1.29, 400: 1.69}.get(n_rep)
     return {"n_rep": n_rep, "flavours": len(pids), "points": len(x), "ms": ms, "evaluations_per_s": ev / (ms * 1e-3),
-            "algorithmic_bytes": bytes_alg, "hbm_gbs": bytes_alg / (ms * 1e-3) / 1e9,
+            "algorithmic_bytes": bytes_alg, "algorithmic_gbs": bytes_alg / t / 1e9, "roofline": roof,
             "paper_pdfflow_gpu_s": paper, "paper_hardware": "system P1 (Titan V / RTX 2080 Ti), PAPER.md:179-188: context, another machine",
             "workload": "synthetic member tables on the NNPDF-shaped knots (workloads.member_values)"}
 
@@ -340,7 +403,7 @@ def run_gpu(args):
     n = args.points
     h = B.load_pdf_spec(grid, device=local)
     # every rank draws its own shard (seed offset by rank): weak scaling, no collective
-    x_h, q2_h = W.queries_in_range(grid, n, 3 + 100 * rank)
+    x_h, q2_h = W.queries_in_range(grid, n, sharding.rank_seed(3, rank))
     x_d, q2_d = torch.from_numpy(x_h).cuda(), torch.from_numpy(q2_h).cuda()
     out_d = torch.empty((F, n), dtype=torch.float64, device="cuda")
 
@@ -372,19 +435,16 @@ def run_gpu(args):
     total_ms = t0.elapsed_time(t1)
     per_step = sorted(a.elapsed_time(b) for a, b in evs)
     kern_ms, kern_med, kern_best = float(np.mean(per_step)), float(np.median(per_step)), per_step[0]
-    if dist is not None:
-        t = torch.tensor([total_ms, kern_ms, kern_med, kern_best], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms, kern_ms, kern_med, kern_best = (float(v) for v in t)
+    total_ms, kern_ms, kern_med, kern_best = sharding.reduce_max([total_ms, kern_ms, kern_med, kern_best], dist, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * n * F / (ms_per_step * 1e-3)
+    value = sharding.aggregate_throughput([n * F] * world, [ms_per_step])
 
     # ---- end to end: pinned host buffers through pdf_xfxq2_host, copies inside the timed region.
     # Every rank takes part (the value is the whole job's); the pinned buffers of all ranks together
     # stay at one config-3 batch (10.4 GB), whatever the rank count.
     e2e = None
     if not args.no_e2e:
-        n_e = min(n, max(1, args.e2e_points // world))
+        n_e, n_e_all = sharding.e2e_split(args.e2e_points, rank, world, n)
         xp = torch.from_numpy(x_h[:n_e]).pin_memory(); qp = torch.from_numpy(q2_h[:n_e]).pin_memory()
         op = torch.empty((F, n_e), dtype=torch.float64).pin_memory()
         B.pdf_xfxq2_host(h, pids, xp, qp, op)
@@ -395,12 +455,9 @@ def run_gpu(args):
             B.pdf_xfxq2_host(h, pids, xp, qp, op)  # synchronous: returns when `out` is complete
         barrier()
         e_s = (time.perf_counter() - tw) / ks
-        if dist is not None:
-            t = torch.tensor([e_s], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_s = float(t[0])
-        e2e = {"value": world * n_e * F / e_s, "unit": UNIT, "h2d_bytes_per_step": 16 * n_e * world,
-               "d2h_bytes_per_step": 8 * F * n_e * world, "points_per_step": n_e * world, "ms_per_step": e_s * 1e3,
+        e_s = sharding.reduce_max_ms(e_s * 1e3, dist, "cuda") * 1e-3
+        e2e = {"value": sharding.aggregate_throughput([n_e_all * F], [e_s * 1e3]), "unit": UNIT, "h2d_bytes_per_step": 16 * n_e_all,
+               "d2h_bytes_per_step": 8 * F * n_e_all, "points_per_step": n_e_all, "ms_per_step": e_s * 1e3,
                "api": "pdf_xfxq2_host (pinned host buffers, 3-stage copy/compute pipeline)"}
         del xp, qp, op
 
@@ -432,8 +489,8 @@ def run_gpu(args):
                        "grid_setup_ms": B.pdf_grid_setup_ms(h)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": (NCU_TRAFFIC_BYTES_PER_POINT * n / 1e9) if F == 11 else None, "traffic_unit": "GB per launch",
-                         "traffic_source": NCU_TRAFFIC_SOURCE,
+                         "traffic": (ncu_traffic()[0] * n / 1e9) if F == 11 and ncu_traffic()[0] else None, "traffic_unit": "GB per launch",
+                         "traffic_source": ncu_traffic()[1],
                          "kernel": "k_xfxq2_smem" if B.pdf_grid_uses_smem_path(h) else "k_xfxq2_v0", "kernel_ms": kern_ms,
                          "kernel_ms_median": kern_med, "kernel_ms_best": kern_best,
                          "algorithmic_bytes_per_point": 16 + 8 * F, "peak_source": peak_src,
@@ -460,9 +517,12 @@ def run_gpu(args):
         line["other_configs"] = bench_other_configs(torch, B, h, ha, grid, peak, fma_ps, graph=not args.no_graph)
     B.alphas_grid_free(ha)
     if not args.no_members:
-        line["multi_member"] = bench_members(torch, B, local, args.members)
+        line["multi_member"] = bench_members(torch, B, local, args.members, peak, lds_bps, fma_ps)
     if not args.no_cpu_baseline and world == 1:
         line["cpu_baseline"] = cpu_baseline(grid, x_h, q2_h, pids)
+        if not args.no_other_configs:
+            for name, e in cpu_baseline_other_configs(grid).items():
+                line["other_configs"][name]["cpu_baseline"] = e
     if args.parity:
         step()
         torch.cuda.synchronize()
